@@ -1,0 +1,342 @@
+"""Pins of the oracle's step, norm and energy against what the paper and the mathematics fix
+(SURVEY.md 8(c) pin table).  None of the expected values below comes from the oracle or the CUDA path.
+"""
+import os
+
+import numpy as np
+import pytest
+from scipy.linalg import expm
+
+import oracle as orc
+
+SX = np.array([[0, 1], [1, 0]], dtype=complex)
+SZ = np.array([[1, 0], [0, -1]], dtype=complex)
+I2 = np.eye(2, dtype=complex)
+
+
+def rel_l2(a, b):
+    return np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel())
+
+
+# ---------------------------------------------------------------- SU(2) closed form
+@pytest.mark.parametrize("imag", [0, 1])
+def test_su2_against_generic_matrix_exponential(imag):
+    r = np.random.default_rng(5 + imag)
+    cases = [(r.uniform(-3, 3), r.uniform(-2, 2), r.uniform(-2, 2), r.uniform(-1, 1)) for _ in range(200)]
+    cases += [(0.7, 0.0, 0.0, 0.3), (0.7, 0.0, 0.0, -0.3), (-1.2, 1e-9, 0.0, 0.5), (0.3, 0.0, 1e-10, -0.5),
+              (0.0, 2.0, 0.0, 0.25), (0.0, 0.0, 1.5, -0.25), (5.0, 3.0, -4.0, 1e-4)]
+    for a, bx, bz, tau in cases:
+        H = a * I2 + bx * SX + bz * SZ
+        ref = expm(-H * tau) if imag else expm(-1j * H * tau)
+        got = orc.su2(a, bx, bz, tau, imag)
+        assert np.abs(got - ref).max() < 1e-11 * max(1.0, np.abs(ref).max()), (a, bx, bz, tau)
+
+
+def test_half_step_wiring_of_g_delta_omega_per_point():
+    """R(tau) at each point = expm(-i H_loc tau) with H_loc from Eqs. 6-8."""
+    r = np.random.default_rng(11)
+    ny, nx = 3, 5
+    psi = r.standard_normal((ny, nx, 2)) + 1j * r.standard_normal((ny, nx, 2))
+    V, Om, de = r.uniform(0, 3, (ny, nx)), r.uniform(-2, 2, (ny, nx)), r.uniform(-1, 1, (ny, nx))
+    g_uu, g_dd, g_ud = 1.3, 0.7, 0.4
+    p = orc.params(nx, ny, 1.0, 1.0, g_uu, g_dd, g_ud)
+    for imag, tau in ((0, 0.037), (0, -0.02), (1, 0.05)):
+        got = orc.half(psi, V, Om, de, p, tau, imag)
+        for iy in range(ny):
+            for ix in range(nx):
+                u, d = psi[iy, ix]
+                nu, nd = abs(u) ** 2, abs(d) ** 2
+                H = np.array([[V[iy, ix] + g_uu * nu + g_ud * nd + de[iy, ix] / 2, Om[iy, ix] / 2],
+                              [Om[iy, ix] / 2, V[iy, ix] + g_dd * nd + g_ud * nu - de[iy, ix] / 2]])
+                U = expm(-H * tau) if imag else expm(-1j * H * tau)
+                np.testing.assert_allclose(got[iy, ix], U @ psi[iy, ix], rtol=0, atol=1e-12)
+    # NULL fields mean zero
+    np.testing.assert_allclose(orc.half(psi, None, None, None, p, 0.01, 0),
+                               orc.half(psi, 0 * V, 0 * Om, 0 * de, p, 0.01, 0), atol=1e-15)
+
+
+# ---------------------------------------------------------------- exact plane wave (signs, k order, recoil, g, delta)
+@pytest.mark.parametrize("mx,my", [(3, -2), (-7, 5), (0, 0), (16, 1)])
+def test_plane_wave_is_exact_under_the_split_step(mx, my):
+    """psi_c = A_c e^{i(kx x + ky y)}, Omega = 0, V const:  psi_c(t) = psi_c(0) e^{-i w_c t},
+    w_up = K_up(k) + V + delta/2 + g_uu|A_up|^2 + g_ud|A_dn|^2 (down alike); exact, not O(dt^2).
+    K_up = ((kx + k_L)^2 + ky^2)/2, K_dn = ((kx - k_L)^2 + ky^2)/2 (reading R-2)."""
+    nx, ny, Lx, Ly = 32, 64, 10.0, 14.0
+    g_uu, g_dd, g_ud, k_L = 0.8, 1.1, 0.35, 1.25
+    V0, d0 = 0.6, -0.4
+    A = np.array([0.7 * np.exp(0.3j), 0.45 * np.exp(-1.1j)])
+    x = -Lx / 2 + Lx / nx * np.arange(nx)
+    y = -Ly / 2 + Ly / ny * np.arange(ny)
+    X, Y = np.meshgrid(x, y)
+    kx, ky = 2 * np.pi * mx / Lx, 2 * np.pi * my / Ly
+    pw = np.exp(1j * (kx * X + ky * Y))
+    psi0 = pw[:, :, None] * A[None, None, :]
+    p = orc.params(nx, ny, Lx, Ly, g_uu, g_dd, g_ud, k_L)
+    V = np.full((ny, nx), V0)
+    de = np.full((ny, nx), d0)
+    n, dt = 1000, 2e-3
+    out = orc.step(psi0, V, None, de, p, n, dt, 0)
+    w_up = ((kx + k_L) ** 2 + ky ** 2) / 2 + V0 + d0 / 2 + g_uu * abs(A[0]) ** 2 + g_ud * abs(A[1]) ** 2
+    w_dn = ((kx - k_L) ** 2 + ky ** 2) / 2 + V0 - d0 / 2 + g_dd * abs(A[1]) ** 2 + g_ud * abs(A[0]) ** 2
+    ref = psi0 * np.exp(-1j * np.array([w_up, w_dn]) * n * dt)[None, None, :]
+    assert np.abs(out - ref).max() < 2e-12
+
+
+def test_single_component_nlse_dispersion_of_eq1():
+    """PAPER.md L51 Eq. (1) with a = 1/2: w = a k^2 + b + c|A|^2 (BASELINE.json north_star)."""
+    n, L = 64, 2 * np.pi
+    x = -L / 2 + L / n * np.arange(n)
+    X, Y = np.meshgrid(x, x)
+    k, b, c, A = 5.0, 0.3, -1.7, 0.9
+    psi0 = np.zeros((n, n, 2), complex)
+    psi0[:, :, 0] = A * np.exp(1j * k * X)
+    p = orc.params(n, n, L, L, g_uu=c)
+    out = orc.step(psi0, np.full((n, n), b), None, None, p, 300, 1e-3, 0)
+    w = 0.5 * k * k + b + c * A * A
+    assert np.abs(out[:, :, 0] - psi0[:, :, 0] * np.exp(-1j * w * 0.3)).max() < 1e-12
+    assert np.abs(out[:, :, 1]).max() == 0.0
+
+
+# ---------------------------------------------------------------- Rabi oscillation (Raman / detuning wiring, the -i)
+@pytest.mark.parametrize("Om,de", [(2.0, 0.0), (1.5, 0.8), (0.9, -2.0)])
+def test_rabi_populations(Om, de):
+    n, L = 16, 4.0
+    psi0 = np.zeros((n, n, 2), complex)
+    psi0[:, :, 0] = 0.5
+    p = orc.params(n, n, L, L)
+    steps, dt = 400, 5e-3
+    t = steps * dt
+    out = orc.step(psi0, None, np.full((n, n), Om), np.full((n, n), de), p, steps, dt, 0)
+    Oeff = np.hypot(Om, de)
+    P_dn = Om ** 2 / Oeff ** 2 * np.sin(Oeff * t / 2) ** 2
+    np.testing.assert_allclose(np.abs(out[:, :, 1]) ** 2 / 0.25, P_dn, rtol=0, atol=1e-13)
+    np.testing.assert_allclose(np.abs(out[:, :, 0]) ** 2 / 0.25, 1 - P_dn, rtol=0, atol=1e-13)
+    if de == 0.0:
+        np.testing.assert_allclose(out[:, :, 1], -1j * np.sin(Om * t / 2) * 0.5, atol=1e-13)
+        np.testing.assert_allclose(out[:, :, 0], np.cos(Om * t / 2) * 0.5, atol=1e-13)
+
+
+# ---------------------------------------------------------------- Eq. 11: minima of the lower Raman band
+def test_eq11_band_minima_from_the_oracle_tables(golden_dir):
+    rows = [l.split() for l in open(os.path.join(golden_dir, "eq11_minima.txt")) if l.strip() and l[0] != "#"]
+    nx, Lx, k_L = 4096, 2 * np.pi * 256, 1.0  # dk = 1/256
+    p = orc.params(nx, 4, Lx, 1.0, k_L=k_L)
+    Kxu, Kxd, Ky = orc.kinetic_tables(p)
+    kx = orc.kgrid(nx, Lx)
+    assert Ky[0] == 0.0
+    for Om_s, kmin_s in rows:
+        Om, kmin = float(Om_s), float(kmin_s)
+        # lower eigenvalue of [[K_up, Om/2], [Om/2, K_dn]] (delta = 0)
+        lower = 0.5 * (Kxu + Kxd) - np.sqrt(0.25 * (Kxu - Kxd) ** 2 + 0.25 * Om ** 2)
+        for sgn in (+1, -1):
+            sel = np.where(sgn * kx > 0)[0]
+            k_at = kx[sel[np.argmin(lower[sel])]]
+            assert abs(abs(k_at) - kmin) <= 1 / 256 + 1e-5, (Om, k_at)
+    # Omega -> 0: up has its minimum at -k_L, down at +k_L
+    assert abs(kx[np.argmin(Kxu)] + k_L) < 1e-12 and abs(kx[np.argmin(Kxd)] - k_L) < 1e-12
+    assert abs(Kxu.min()) < 1e-20  # completed square (R-3)
+
+
+# ---------------------------------------------------------------- energy functional
+def _gauss_setup(n=64, L=16.0):
+    x = -L / 2 + L / n * np.arange(n)
+    X, Y = np.meshgrid(x, x)
+    return X, Y, 0.5 * (X * X + Y * Y)
+
+
+def test_energy_of_the_harmonic_ground_state_is_hbar_omega():
+    X, Y, V = _gauss_setup()
+    psi = np.zeros((64, 64, 2), complex)
+    psi[:, :, 0] = np.exp(-0.5 * (X * X + Y * Y))
+    psi[:, :, 1] = 0.5j * psi[:, :, 0]
+    p = orc.params(64, 64, 16.0, 16.0)
+    N = orc.norm(psi, p)
+    np.testing.assert_allclose(N, [np.pi, np.pi / 4], rtol=1e-13)  # integral of e^{-r^2}
+    E = orc.energy(psi, V, None, None, p)
+    assert abs(E[0] / N.sum() - 1.0) < 1e-13
+    assert abs(E[1] / N.sum() - 0.5) < 1e-13 and abs(E[2] / N.sum() - 0.5) < 1e-13
+    assert E[3] == 0.0 and E[4] == 0.0
+
+
+def test_energy_of_a_uniform_two_component_state_closed_form():
+    nx, ny, Lx, Ly = 16, 32, 3.0, 5.0
+    g_uu, g_dd, g_ud, k_L = 1.3, 0.6, 0.9, 0.7
+    V0, Om0, d0 = 0.4, 1.1, -0.3
+    a, b = 0.8 * np.exp(0.4j), 0.5 * np.exp(-0.9j)
+    psi = np.empty((ny, nx, 2), complex)
+    psi[:, :, 0], psi[:, :, 1] = a, b
+    p = orc.params(nx, ny, Lx, Ly, g_uu, g_dd, g_ud, k_L)
+    E = orc.energy(psi, np.full((ny, nx), V0), np.full((ny, nx), Om0), np.full((ny, nx), d0), p)
+    A = Lx * Ly
+    nu, nd = abs(a) ** 2, abs(b) ** 2
+    kin = A * 0.5 * k_L ** 2 * (nu + nd)  # k = 0 mode: K_up = K_dn = k_L^2/2
+    pot = A * (V0 * (nu + nd) + 0.5 * d0 * (nu - nd))
+    inter = A * (0.5 * g_uu * nu ** 2 + 0.5 * g_dd * nd ** 2 + g_ud * nu * nd)
+    ram = A * Om0 * (np.conj(a) * b).real
+    np.testing.assert_allclose(E[1:], [kin, pot, inter, ram], rtol=1e-12)
+    assert abs(E[0] - (kin + pot + inter + ram)) < 1e-12 * abs(E[0])
+
+
+def test_energy_and_norm_conservation_in_real_time():
+    """A wrong 1/2 in the interaction energy or a wrong Raman term breaks conservation."""
+    n, L = 64, 16.0
+    X, Y, V = _gauss_setup(n, L)
+    psi = np.zeros((n, n, 2), complex)
+    psi[:, :, 0] = np.exp(-0.3 * ((X - 0.5) ** 2 + Y * Y))
+    psi[:, :, 1] = 0.6 * np.exp(-0.4 * (X * X + (Y + 0.3) ** 2)) * np.exp(0.5j * X)
+    p = orc.params(n, n, L, L, 2.0, 1.5, 1.0, 0.8)
+    Om, de = 1.2 * np.tanh(Y), 0.3 * X
+    E0, N0 = orc.energy(psi, V, Om, de, p), orc.norm(psi, p)
+    assert E0[3] > 0.1 * abs(E0[0]) and abs(E0[4]) > 0.01 * abs(E0[0])  # both terms matter here
+    out = orc.step(psi, V, Om, de, p, 400, 5e-4, 0)
+    E1, N1 = orc.energy(out, V, Om, de, p), orc.norm(out, p)
+    assert abs(N1.sum() - N0.sum()) < 1e-12 * N0.sum()
+    assert abs(E1[0] - E0[0]) < 2e-6 * abs(E0[0])
+    assert abs(E1[3] - E0[3]) > 1e-4 * abs(E0[0])  # the parts do move; only the sum is conserved
+    # halving dt quarters the (bounded, O(dt^2)) energy error
+    out2 = orc.step(psi, V, Om, de, p, 800, 2.5e-4, 0)
+    e1 = abs(E1[0] - E0[0])
+    e2 = abs(orc.energy(out2, V, Om, de, p)[0] - E0[0])
+    assert e2 < 0.6 * e1
+
+
+# ---------------------------------------------------------------- imaginary time
+def test_imaginary_time_ground_state_is_stationary_and_excited_state_decays_as_exp_minus_tau():
+    n, L = 64, 16.0
+    X, Y, V = _gauss_setup(n, L)
+    phi0 = np.exp(-0.5 * (X * X + Y * Y))
+    phi1 = X * phi0  # first excited state, E1 - E0 = 1
+    p = orc.params(n, n, L, L)
+    psi = np.zeros((n, n, 2), complex)
+    psi[:, :, 0] = phi0
+    psi[:, :, 1] = phi0 + 0.1 * phi1
+    out = orc.step(psi, V, None, None, p, 200, 1e-3, 1)
+    # component 0: stationary up to the O(dt^2) Strang fixed point
+    assert rel_l2(out[:, :, 0], psi[:, :, 0]) < 1e-6
+    np.testing.assert_allclose(orc.norm(out, p), orc.norm(psi, p), rtol=1e-13)  # renormalised to targets
+    E = orc.energy(np.stack([out[:, :, 0], 0 * out[:, :, 0]], -1), V, None, None, p)
+    assert abs(E[0] / orc.norm(out, p)[0] - 1.0) < 1e-9
+    # component 1: ratio of projections c1/c0 decays by e^{-(E1-E0) tau} = e^{-0.2}
+    c0 = lambda f: np.sum(phi0 * f).real / np.sum(phi0 * phi0)
+    c1 = lambda f: np.sum(phi1 * f).real / np.sum(phi1 * phi1)
+    r_before = c1(psi[:, :, 1]) / c0(psi[:, :, 1])
+    r_after = c1(out[:, :, 1]) / c0(out[:, :, 1])
+    assert abs(r_after / r_before - np.exp(-0.2)) < 1e-6
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_imaginary_time_normalisation_modes(mode):
+    n, L = 32, 12.0
+    X, Y, V = _gauss_setup(n, L)
+    r = np.random.default_rng(2)
+    psi = (np.exp(-0.4 * (X * X + Y * Y))[:, :, None] * (1 + 0.1 * r.standard_normal((n, n, 2)))).astype(complex)
+    p = orc.params(n, n, L, L, 1.0, 1.0, 0.5, norm_mode=mode)
+    Om = np.full((n, n), 1.5)
+    N0 = orc.norm(psi, p)
+    out = orc.step(psi, V, Om, None, p, 20, 5e-3, 1)
+    N1 = orc.norm(out, p)
+    if mode == 0:
+        np.testing.assert_allclose(N1, N0, rtol=1e-13)
+    else:
+        assert abs(N1.sum() - N0.sum()) < 1e-13 * N0.sum()
+        assert abs(N1[0] - N0[0]) > 1e-6  # components exchange population through Omega
+    # explicit targets
+    out2 = orc.step(psi, V, Om, None, p, 3, 5e-3, 1, targets=[2.0, 3.0])
+    N2 = orc.norm(out2, p)
+    if mode == 0:
+        np.testing.assert_allclose(N2, [2.0, 3.0], rtol=1e-13)
+    else:
+        assert abs(N2.sum() - 5.0) < 1e-12
+
+
+def test_config1_end_to_end_reaches_hbar_omega():
+    from workloads import make_workload
+    w = make_workload(1)
+    p = orc.params_of(w)
+    psi = w.psi0
+    np.testing.assert_allclose(orc.norm(psi, p), [0.5, 0.5], rtol=1e-13)
+    for (n, dt, imag) in w.schedule:
+        if imag:
+            psi = orc.step(psi, w.V, w.Omega, w.delta, p, n, dt, imag)
+            E = orc.energy(psi, w.V, None, None, p)
+            assert abs(E[0] / orc.norm(psi, p).sum() - 1.0) < 1e-5
+        else:
+            E0, N0 = orc.energy(psi, w.V, None, None, p)[0], orc.norm(psi, p)
+            psi = orc.step(psi, w.V, w.Omega, w.delta, p, n, dt, imag)
+            np.testing.assert_allclose(orc.norm(psi, p), N0, rtol=1e-12)
+            assert abs(orc.energy(psi, w.V, None, None, p)[0] - E0) < 1e-9 * abs(E0)
+
+
+# ---------------------------------------------------------------- reversibility, order, brute force
+def _small_problem(g, Om_amp):
+    n, L = 32, 12.0
+    X, Y, V = _gauss_setup(n, L)
+    psi = np.zeros((n, n, 2), complex)
+    psi[:, :, 0] = np.exp(-0.35 * ((X - 0.4) ** 2 + Y * Y)) * np.exp(0.3j * Y)
+    psi[:, :, 1] = 0.7 * np.exp(-0.45 * (X * X + (Y + 0.2) ** 2))
+    p = orc.params(n, n, L, L, g[0], g[1], g[2], 0.6)
+    Om = Om_amp * np.tanh(Y / 2.0) + 0.5 * Om_amp
+    de = 0.2 * X
+    return psi, V, Om, de, p
+
+
+def test_reversibility():
+    """step(n, dt) then step(n, -dt) returns the input when the g's are equal or Omega = 0 (R-5, R-6);
+    with Omega != 0 and unequal g the frozen-density exponential is only first order and does not."""
+    for g, Om_amp, reversible in (((2.0, 2.0, 2.0), 3.0, True), ((2.0, 1.0, 0.5), 0.0, True),
+                                  ((2.0, 1.0, 0.5), 3.0, False)):
+        psi, V, Om, de, p = _small_problem(g, Om_amp)
+        fwd = orc.step(psi, V, Om, de, p, 100, 2e-3, 0)
+        back = orc.step(fwd, V, Om, de, p, 100, -2e-3, 0)
+        err = rel_l2(back, psi)
+        assert rel_l2(fwd, psi) > 1e-2
+        if reversible:
+            assert err < 1e-12, (g, Om_amp, err)
+        else:
+            assert 1e-9 < err < 1e-3, (g, Om_amp, err)
+
+
+def test_order_of_convergence():
+    """dt halving against a fine reference: order 2 when Omega = 0 or the g's are equal; lower otherwise (R-5)."""
+    def order(g, Om_amp):
+        psi, V, Om, de, p = _small_problem(g, Om_amp)
+        T = 0.128
+        ref = orc.step(psi, V, Om, de, p, 2048, T / 2048, 0)
+        e = [rel_l2(orc.step(psi, V, Om, de, p, n, T / n, 0), ref) for n in (16, 32, 64)]
+        return np.log2(e[0] / e[1]), np.log2(e[1] / e[2])
+    for g, Om_amp in (((2.0, 2.0, 2.0), 3.0), ((2.0, 1.0, 0.5), 0.0)):
+        o = order(g, Om_amp)
+        assert 1.9 < o[0] < 2.1 and 1.9 < o[1] < 2.1, (g, Om_amp, o)
+    o = order((8.0, 1.0, 0.5), 3.0)
+    assert o[1] < 1.9, o
+
+
+@pytest.mark.parametrize("n", [4, 8, 16])
+def test_whole_step_naive_dft_path_equals_radix2_path(n):
+    r = np.random.default_rng(n)
+    psi = r.standard_normal((n, 2 * n, 2)) + 1j * r.standard_normal((n, 2 * n, 2))
+    V, Om, de = r.uniform(0, 2, (n, 2 * n)), r.uniform(-1, 1, (n, 2 * n)), r.uniform(-1, 1, (n, 2 * n))
+    kw = dict(g_uu=1.0, g_dd=0.8, g_ud=0.3, k_L=0.9)
+    for imag in (0, 1):
+        a = orc.step(psi, V, Om, de, orc.params(2 * n, n, 5.0, 4.0, naive_max=64, **kw), 3, 1e-2, imag)
+        b = orc.step(psi, V, Om, de, orc.params(2 * n, n, 5.0, 4.0, naive_max=0, **kw), 3, 1e-2, imag)
+        assert rel_l2(a, b) < 1e-13
+
+
+def test_kinetic_step_free_gaussian_spreading():
+    """Linear limit c -> 0: free 1-D-in-x Gaussian e^{-x^2/2} under i dpsi/dt = -(1/2) d2psi/dx2
+    becomes (1+it)^{-1/2} e^{-x^2/(2(1+it))}; checks the kinetic factor, its sign and the k grid."""
+    nx, ny, Lx, Ly = 256, 4, 40.0, 1.0
+    x = -Lx / 2 + Lx / nx * np.arange(nx)
+    psi = np.zeros((ny, nx, 2), complex)
+    psi[:, :, 0] = np.exp(-0.5 * x * x)[None, :]
+    psi[:, :, 1] = psi[:, :, 0]
+    p = orc.params(nx, ny, Lx, Ly)
+    t = 0.7
+    out = orc.kinetic(psi, p, t, 0)
+    ref = (1 + 1j * t) ** -0.5 * np.exp(-0.5 * x * x / (1 + 1j * t))
+    assert np.abs(out[0, :, 0] - ref).max() < 1e-12
+    # imaginary time: heat kernel, (1+t)^{-1/2} e^{-x^2/(2(1+t))}
+    out = orc.kinetic(psi, p, t, 1)
+    ref = (1 + t) ** -0.5 * np.exp(-0.5 * x * x / (1 + t))
+    assert np.abs(out[1, :, 1] - ref).max() < 1e-12
