@@ -1,0 +1,112 @@
+/*
+ * spgpe.h -- C ABI of libspgpe: the Strang time-splitting spectral step for the quasi-2D
+ * two-component (pseudospinor) Gross-Pitaevskii equation of arXiv 2010.15069, on one NVIDIA
+ * B200 (sm_100a).  Every step of the path runs in the library's own CUDA kernels; there is no
+ * cuFFT, no CPU fallback and no host synchronisation inside spgpe_step.
+ *
+ * Citations: "P:Lnnn" = line of the paper text; "R-n" = reading n in DESIGN.md
+ * section "Readings of the paper".
+ *
+ * Model (Eqs. 4-8, sign convention R-1):  i d/dt Psi = H Psi,  Psi = (psi_up, psi_dn),
+ *   H = K + V(r) + (delta(r)/2) sigma_z + (Omega(r)/2) sigma_x + diag(g_uu n_up + g_ud n_dn, g_dd n_dn + g_ud n_up),
+ *   K_up = ((k_x + k_L)^2 + k_y^2)/2,  K_dn = ((k_x - k_L)^2 + k_y^2)/2   (Eq. 5, R-2, R-3),  n_c = |psi_c|^2.
+ * One step of size dt (Eq. 9, operator order R-4):
+ *   Psi <- R(dt/2) F^-1 exp(-i K dt) F R(dt/2) Psi,
+ * R(tau) = per-point 2x2 exponential exp(-i tau H_loc) in closed SU(2) form with the densities of the
+ * Psi entering it (R-5, R-6).  Imaginary time replaces exp(-i . ) by exp(- . ) and
+ * renormalises after every step (R-7).
+ *
+ * Layout.  Grid nx x ny, box [-Lx/2, Lx/2) x [-Ly/2, Ly/2) (R-9), x fastest:
+ *   psi   : complex [ny][nx][2], component 0 = up, 1 = down, interleaved per point; one element is
+ *           (re, im) of the working precision: 2 doubles (SPGPE_C128) or 2 floats (SPGPE_C64).
+ *   fields: real [ny][nx] of the working precision (double or float); V, Omega, delta.
+ * All sizes are in elements of that layout; nothing is padded.
+ *
+ * Pointers.  Arguments named d_* are DEVICE pointers, h_* are HOST pointers.  All arrays are owned by
+ * the caller; set_* calls copy into library-owned storage (the caller's buffer may be reused once the
+ * stream has passed that point), get_* calls copy out.  The handle owns psi, the three fields, the
+ * tables and the reduction scratch.
+ *
+ * Errors.  Every call returns SPGPE_OK (0) or a negative code; nothing is printed, nothing aborts.
+ * spgpe_step only enqueues work on the handle's stream; asynchronous kernel errors surface at the next
+ * synchronising call (spgpe_norm, spgpe_energy, spgpe_get_psi_host, spgpe_synchronize).
+ * NaN/Inf are propagated, not trapped.
+ */
+#ifndef SPGPE_H
+#define SPGPE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct spgpe_ctx* spgpe_handle; /* opaque */
+
+enum { SPGPE_C128 = 0, SPGPE_C64 = 1 }; /* storage precision of psi and fields (arithmetic is fp64) */
+enum { SPGPE_NORM_PER_COMPONENT = 0, SPGPE_NORM_TOTAL = 1 }; /* R-7 */
+
+enum {
+  SPGPE_OK = 0,
+  SPGPE_ERR_INVALID_ARG = -1, /* NULL handle/pointer, non-positive size, unknown enum */
+  SPGPE_ERR_UNSUPPORTED = -2, /* nx or ny not a power of two in [64, 4096] */
+  SPGPE_ERR_NOT_READY = -3,   /* step/norm/energy/get before set_psi */
+  SPGPE_ERR_CUDA = -4,        /* a CUDA call failed; spgpe_last_cuda_error() gives its text */
+  SPGPE_ERR_NO_DEVICE = -5    /* no CUDA device / not an sm_100 device */
+};
+
+typedef struct {
+  int dtype;               /* SPGPE_C128 | SPGPE_C64 */
+  double g_uu, g_dd, g_ud; /* Eq. 7 */
+  double k_L;              /* signed recoil wavenumber along x, Eq. 5, R-2; 0 disables the shift */
+  int norm_mode;           /* imaginary-time renormalisation rule, R-7 */
+} spgpe_params;
+
+/* Create a solver for an nx x ny grid on the box of full widths Lx, Ly.  cuda_stream is a cudaStream_t
+ * (NULL = the default stream); all work of the handle is enqueued on it.  Fields start as zero. */
+int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double Ly, const spgpe_params* p,
+                 void* cuda_stream);
+int spgpe_destroy(spgpe_handle h);
+
+/* Fields of Eqs. 6 and 8: trap V(r), Raman coupling Omega(r) (real, R-11), Zeeman
+ * detuning delta(r).  real [ny][nx]; NULL = zero everywhere. */
+int spgpe_set_potential(spgpe_handle h, const void* d_V);
+int spgpe_set_raman(spgpe_handle h, const void* d_Omega);
+int spgpe_set_zeeman(spgpe_handle h, const void* d_delta);
+int spgpe_set_potential_host(spgpe_handle h, const void* h_V);
+int spgpe_set_raman_host(spgpe_handle h, const void* h_Omega);
+int spgpe_set_zeeman_host(spgpe_handle h, const void* h_delta);
+
+/* Order parameter in / out ("initial order parameter in, final order parameter available").
+ * set_psi also captures the imaginary-time norm targets N_up, N_dn of the given state (R-7). */
+int spgpe_set_psi(spgpe_handle h, const void* d_psi);
+int spgpe_get_psi(spgpe_handle h, void* d_psi);
+int spgpe_set_psi_host(spgpe_handle h, const void* h_psi); /* synchronous w.r.t. the host buffer */
+int spgpe_get_psi_host(spgpe_handle h, void* h_psi);       /* synchronises the stream */
+int spgpe_set_norm_targets(spgpe_handle h, double n_up, double n_dn);
+
+/* n Strang steps of size dt.  imag != 0: imaginary time with dt = d tau > 0 and a
+ * renormalisation after every step.  dt may be negative in real time.  Asynchronous.
+ * step(n) then step(m) equals step(n+m) to rounding. */
+int spgpe_step(spgpe_handle h, int n, double dt, int imag);
+
+/* N_c = dx dy sum_r |psi_c|^2 (R-8); out = {N_up, N_dn}; synchronises. */
+int spgpe_norm(spgpe_handle h, double out[2]);
+/* Energy functional implied by Eqs. 4-8 (R-8), totals not per particle:
+ * out = {total, kinetic, potential+Zeeman, interaction, Raman}; synchronises. */
+int spgpe_energy(spgpe_handle h, double out[5]);
+
+int spgpe_synchronize(spgpe_handle h);
+/* Number of kernels the handle has launched so far (bench.py's gpu_launches claim). */
+long long spgpe_launch_count(spgpe_handle h);
+const char* spgpe_strerror(int code);
+const char* spgpe_last_cuda_error(void);
+
+/* Measurement helpers (not part of the method): peak probes used for bench.py's roofline denominators.
+ * spgpe_probe_dfma: sustained fp64 FMA rate of the device in TFLOP/s (2 flops per FMA).
+ * spgpe_probe_copy: device-to-device copy bandwidth in GB/s (read + write bytes) over `bytes` bytes. */
+int spgpe_probe_dfma(void* cuda_stream, double* tflops);
+int spgpe_probe_copy(void* cuda_stream, long long bytes, double* gbs);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPGPE_H */

@@ -1,0 +1,361 @@
+// api.cu -- the C ABI of include/spgpe.h: handle, uploads, step orchestration, norm, energy.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "../../include/spgpe.h"
+#include "internal.h"
+
+using namespace spgpe;
+
+struct spgpe_ctx {
+  int nx, ny;
+  double Lx, Ly;
+  spgpe_params p;
+  cudaStream_t stream;
+  int dt;  // storage precision
+  size_t points, field_bytes, psi_bytes;
+  void* psi;
+  void* scratch;  // second psi buffer, allocated by the first spgpe_energy
+  void *Vbuf, *Ombuf, *Debuf;  // owned storage
+  const void *V, *Om, *De;     // NULL = zero field
+  double2 *tw_x, *tw_y;
+  double *Kx, *Ky;       // kinetic tables in stored order: Kx[2][nx], Ky[ny]
+  double2 *exk, *eyk;    // phase tables of (tab_dt, tab_imag)
+  double tab_dt;
+  int tab_imag;
+  bool tab_valid;
+  double *partial, *scale, *target, *dout;
+  int partial_cap;
+  bool ready;
+  long long launches;
+  HalfCoef hc;
+};
+
+static thread_local char g_cuda_err[256] = "";
+
+static int cuda_fail(cudaError_t e) {
+  snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+  return SPGPE_ERR_CUDA;
+}
+#define CK(call)                                  \
+  do {                                            \
+    cudaError_t e__ = (call);                     \
+    if (e__ != cudaSuccess) return cuda_fail(e__); \
+  } while (0)
+
+static bool size_ok(int n) { return n >= 64 && n <= 4096 && (n & (n - 1)) == 0; }
+
+static cudaError_t dispatch_x(spgpe_ctx* h, int mode, const PassXArgs& a) {
+  h->launches++;
+  switch (h->nx) {
+    case 64: return launch_pass_x_64(h->dt, mode, a, h->ny, h->stream);
+    case 128: return launch_pass_x_128(h->dt, mode, a, h->ny, h->stream);
+    case 256: return launch_pass_x_256(h->dt, mode, a, h->ny, h->stream);
+    case 512: return launch_pass_x_512(h->dt, mode, a, h->ny, h->stream);
+    case 1024: return launch_pass_x_1024(h->dt, mode, a, h->ny, h->stream);
+    case 2048: return launch_pass_x_2048(h->dt, mode, a, h->ny, h->stream);
+    default: return launch_pass_x_4096(h->dt, mode, a, h->ny, h->stream);
+  }
+}
+static cudaError_t dispatch_y(spgpe_ctx* h, int ymode, const PassYArgs& a) {
+  h->launches++;
+  switch (h->ny) {
+    case 64: return launch_pass_y_64(h->dt, ymode, a, h->stream);
+    case 128: return launch_pass_y_128(h->dt, ymode, a, h->stream);
+    case 256: return launch_pass_y_256(h->dt, ymode, a, h->stream);
+    case 512: return launch_pass_y_512(h->dt, ymode, a, h->stream);
+    case 1024: return launch_pass_y_1024(h->dt, ymode, a, h->stream);
+    case 2048: return launch_pass_y_2048(h->dt, ymode, a, h->stream);
+    default: return launch_pass_y_4096(h->dt, ymode, a, h->stream);
+  }
+}
+
+// kinetic tables in the stored order of the transforms (Eq. 5; R-2, R-3, R-9)
+static void fill_ktables(const spgpe_ctx* h, std::vector<double>& Kx, std::vector<double>& Ky) {
+  const double two_pi = 6.283185307179586476925286766559;
+  Kx.resize(2 * (size_t)h->nx);
+  Ky.resize(h->ny);
+  for (int pos = 0; pos < h->nx; ++pos) {
+    const int f = plan_freq_of_pos(h->nx, pos);
+    const int mt = (f < h->nx / 2) ? f : f - h->nx;
+    const double k = two_pi * (double)mt / h->Lx;
+    Kx[pos] = 0.5 * (k + h->p.k_L) * (k + h->p.k_L);
+    Kx[h->nx + pos] = 0.5 * (k - h->p.k_L) * (k - h->p.k_L);
+  }
+  for (int pos = 0; pos < h->ny; ++pos) {
+    const int f = plan_freq_of_pos(h->ny, pos);
+    const int mt = (f < h->ny / 2) ? f : f - h->ny;
+    const double k = two_pi * (double)mt / h->Ly;
+    Ky[pos] = 0.5 * k * k;
+  }
+}
+
+extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double Ly, const spgpe_params* p,
+                            void* cuda_stream) {
+  if (!out || !p || !(Lx > 0.0) || !(Ly > 0.0)) return SPGPE_ERR_INVALID_ARG;
+  if (p->dtype != SPGPE_C128 && p->dtype != SPGPE_C64) return SPGPE_ERR_INVALID_ARG;
+  if (p->norm_mode != SPGPE_NORM_PER_COMPONENT && p->norm_mode != SPGPE_NORM_TOTAL) return SPGPE_ERR_INVALID_ARG;
+  if (!size_ok(nx) || !size_ok(ny)) return SPGPE_ERR_UNSUPPORTED;
+  int dev = 0, ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return SPGPE_ERR_NO_DEVICE;
+  CK(cudaGetDevice(&dev));
+  int major = 0;
+  CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+  if (major != 10) return SPGPE_ERR_NO_DEVICE;
+
+  spgpe_ctx* h = new (std::nothrow) spgpe_ctx();
+  if (!h) return SPGPE_ERR_INVALID_ARG;
+  memset(h, 0, sizeof(*h));
+  h->nx = nx; h->ny = ny; h->Lx = Lx; h->Ly = Ly; h->p = *p;
+  h->stream = (cudaStream_t)cuda_stream;
+  h->dt = p->dtype;
+  h->points = (size_t)nx * ny;
+  const size_t rsz = (h->dt == SPGPE_C128) ? 8 : 4;
+  h->field_bytes = h->points * rsz;
+  h->psi_bytes = h->points * 4 * rsz;
+  h->hc.ca_u = 0.5 * (p->g_uu + p->g_ud);
+  h->hc.ca_d = 0.5 * (p->g_dd + p->g_ud);
+  h->hc.cb_u = 0.5 * (p->g_uu - p->g_ud);
+  h->hc.cb_d = 0.5 * (p->g_ud - p->g_dd);
+  h->partial_cap = 4 * (nx > ny ? nx : ny);
+  if (h->partial_cap < 4 * 2048) h->partial_cap = 4 * 2048;
+
+  cudaError_t e = cudaSuccess;
+  auto alloc = [&](void** ptr, size_t bytes) {
+    if (e == cudaSuccess) e = cudaMalloc(ptr, bytes);
+  };
+  alloc(&h->psi, h->psi_bytes);
+  alloc(&h->Vbuf, h->field_bytes);
+  alloc(&h->Ombuf, h->field_bytes);
+  alloc(&h->Debuf, h->field_bytes);
+  const int twx = plan_tw_total(nx), twy = plan_tw_total(ny);
+  alloc((void**)&h->tw_x, sizeof(double2) * twx);
+  alloc((void**)&h->tw_y, sizeof(double2) * twy);
+  alloc((void**)&h->Kx, sizeof(double) * 2 * nx);
+  alloc((void**)&h->Ky, sizeof(double) * ny);
+  alloc((void**)&h->exk, sizeof(double2) * 2 * nx);
+  alloc((void**)&h->eyk, sizeof(double2) * ny);
+  alloc((void**)&h->partial, sizeof(double) * h->partial_cap);
+  alloc((void**)&h->scale, sizeof(double) * 2);
+  alloc((void**)&h->target, sizeof(double) * 2);
+  alloc((void**)&h->dout, sizeof(double) * 8);
+  if (e == cudaSuccess) {
+    std::vector<double2> tw(twx > twy ? twx : twy);
+    plan_fill_twiddles(nx, tw.data());
+    e = cudaMemcpy(h->tw_x, tw.data(), sizeof(double2) * twx, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+      plan_fill_twiddles(ny, tw.data());
+      e = cudaMemcpy(h->tw_y, tw.data(), sizeof(double2) * twy, cudaMemcpyHostToDevice);
+    }
+  }
+  if (e == cudaSuccess) {
+    std::vector<double> Kx, Ky;
+    fill_ktables(h, Kx, Ky);
+    e = cudaMemcpy(h->Kx, Kx.data(), sizeof(double) * Kx.size(), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(h->Ky, Ky.data(), sizeof(double) * Ky.size(), cudaMemcpyHostToDevice);
+  }
+  if (e != cudaSuccess) {
+    spgpe_destroy(h);
+    return cuda_fail(e);
+  }
+  *out = h;
+  return SPGPE_OK;
+}
+
+extern "C" int spgpe_destroy(spgpe_handle h) {
+  if (!h) return SPGPE_ERR_INVALID_ARG;
+  cudaStreamSynchronize(h->stream);
+  void* ptrs[] = {h->psi, h->scratch, h->Vbuf, h->Ombuf, h->Debuf, h->tw_x, h->tw_y, h->Kx, h->Ky,
+                  h->exk, h->eyk, h->partial, h->scale, h->target, h->dout};
+  for (void* p : ptrs)
+    if (p) cudaFree(p);
+  delete h;
+  return SPGPE_OK;
+}
+
+static int set_field(spgpe_handle h, const void* src, void* buf, const void** slot, cudaMemcpyKind kind) {
+  if (!h) return SPGPE_ERR_INVALID_ARG;
+  if (!src) {
+    *slot = nullptr;
+    return SPGPE_OK;
+  }
+  CK(cudaMemcpyAsync(buf, src, h->field_bytes, kind, h->stream));
+  if (kind == cudaMemcpyHostToDevice) CK(cudaStreamSynchronize(h->stream));
+  *slot = buf;
+  return SPGPE_OK;
+}
+extern "C" int spgpe_set_potential(spgpe_handle h, const void* d) {
+  return h ? set_field(h, d, h->Vbuf, &h->V, cudaMemcpyDeviceToDevice) : SPGPE_ERR_INVALID_ARG;
+}
+extern "C" int spgpe_set_raman(spgpe_handle h, const void* d) {
+  return h ? set_field(h, d, h->Ombuf, &h->Om, cudaMemcpyDeviceToDevice) : SPGPE_ERR_INVALID_ARG;
+}
+extern "C" int spgpe_set_zeeman(spgpe_handle h, const void* d) {
+  return h ? set_field(h, d, h->Debuf, &h->De, cudaMemcpyDeviceToDevice) : SPGPE_ERR_INVALID_ARG;
+}
+extern "C" int spgpe_set_potential_host(spgpe_handle h, const void* p) {
+  return h ? set_field(h, p, h->Vbuf, &h->V, cudaMemcpyHostToDevice) : SPGPE_ERR_INVALID_ARG;
+}
+extern "C" int spgpe_set_raman_host(spgpe_handle h, const void* p) {
+  return h ? set_field(h, p, h->Ombuf, &h->Om, cudaMemcpyHostToDevice) : SPGPE_ERR_INVALID_ARG;
+}
+extern "C" int spgpe_set_zeeman_host(spgpe_handle h, const void* p) {
+  return h ? set_field(h, p, h->Debuf, &h->De, cudaMemcpyHostToDevice) : SPGPE_ERR_INVALID_ARG;
+}
+
+static int norms_to(spgpe_handle h, double* d_out2) {
+  const int nblk = 1024;
+  h->launches += 2;
+  CK(aux_norm_partials(h->dt, h->psi, h->points, h->partial, nblk, h->stream));
+  CK(aux_sum_partials(h->partial, nblk, 2, (h->Lx / h->nx) * (h->Ly / h->ny), d_out2, h->stream));
+  return SPGPE_OK;
+}
+
+static int set_psi_common(spgpe_handle h, const void* src, cudaMemcpyKind kind) {
+  if (!h || !src) return SPGPE_ERR_INVALID_ARG;
+  CK(cudaMemcpyAsync(h->psi, src, h->psi_bytes, kind, h->stream));
+  if (kind == cudaMemcpyHostToDevice) CK(cudaStreamSynchronize(h->stream));
+  h->ready = true;
+  return norms_to(h, h->target);  // R-7: targets are the norms of the state handed in
+}
+extern "C" int spgpe_set_psi(spgpe_handle h, const void* d) { return set_psi_common(h, d, cudaMemcpyDeviceToDevice); }
+extern "C" int spgpe_set_psi_host(spgpe_handle h, const void* p) { return set_psi_common(h, p, cudaMemcpyHostToDevice); }
+
+extern "C" int spgpe_get_psi(spgpe_handle h, void* d) {
+  if (!h || !d) return SPGPE_ERR_INVALID_ARG;
+  if (!h->ready) return SPGPE_ERR_NOT_READY;
+  CK(cudaMemcpyAsync(d, h->psi, h->psi_bytes, cudaMemcpyDeviceToDevice, h->stream));
+  return SPGPE_OK;
+}
+extern "C" int spgpe_get_psi_host(spgpe_handle h, void* p) {
+  if (!h || !p) return SPGPE_ERR_INVALID_ARG;
+  if (!h->ready) return SPGPE_ERR_NOT_READY;
+  CK(cudaMemcpyAsync(p, h->psi, h->psi_bytes, cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return SPGPE_OK;
+}
+extern "C" int spgpe_set_norm_targets(spgpe_handle h, double n_up, double n_dn) {
+  if (!h || !(n_up > 0.0) || !(n_dn > 0.0)) return SPGPE_ERR_INVALID_ARG;
+  h->launches++;
+  CK(aux_set_targets(h->target, n_up, n_dn, h->stream));
+  return SPGPE_OK;
+}
+
+static int ensure_tables(spgpe_handle h, double dt, int imag) {
+  if (h->tab_valid && h->tab_dt == dt && h->tab_imag == imag) return SPGPE_OK;
+  h->launches++;
+  CK(aux_phase_tables(h->Kx, h->Ky, h->nx, h->ny, dt, imag, h->exk, h->eyk, h->stream));
+  h->tab_dt = dt; h->tab_imag = imag; h->tab_valid = true;
+  return SPGPE_OK;
+}
+
+extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
+  if (!h || n < 0 || !(dt == dt)) return SPGPE_ERR_INVALID_ARG;
+  if (!h->ready) return SPGPE_ERR_NOT_READY;
+  if (n == 0) return SPGPE_OK;
+  imag = imag ? 1 : 0;
+  int rc = ensure_tables(h, dt, imag);
+  if (rc) return rc;
+  PassXArgs xa;
+  memset(&xa, 0, sizeof(xa));
+  xa.src = h->psi; xa.dst = h->psi; xa.V = h->V; xa.Om = h->Om; xa.De = h->De;
+  xa.tw = h->tw_x; xa.exk = h->exk; xa.scale = nullptr; xa.partial = h->partial;
+  xa.tau = 0.5 * dt; xa.hc = h->hc; xa.imag = imag; xa.want_norm = imag;
+  PassYArgs ya;
+  memset(&ya, 0, sizeof(ya));
+  ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx;
+  const int xblocks = h->ny / plan_lines(h->nx);
+  const double w = (h->Lx / h->nx) * (h->Ly / h->ny);
+  if (!imag) {
+    CK(dispatch_x(h, MODE_PRO, xa));
+    for (int s = 1; s <= n; ++s) {
+      CK(dispatch_y(h, YMODE_STEP, ya));
+      CK(dispatch_x(h, s < n ? MODE_MID : MODE_EPI, xa));
+    }
+  } else {
+    for (int s = 0; s < n; ++s) {
+      xa.scale = (s > 0) ? h->scale : nullptr;  // rescale of the previous step, applied at load
+      CK(dispatch_x(h, MODE_PRO, xa));
+      CK(dispatch_y(h, YMODE_STEP, ya));
+      CK(dispatch_x(h, MODE_EPI, xa));
+      h->launches++;
+      CK(aux_norm_scale(h->partial, xblocks, w, h->target, h->p.norm_mode, h->scale, h->stream));
+    }
+    h->launches++;
+    CK(aux_apply_scale(h->dt, h->psi, h->points, h->scale, h->stream));
+  }
+  return SPGPE_OK;
+}
+
+extern "C" int spgpe_norm(spgpe_handle h, double out[2]) {
+  if (!h || !out) return SPGPE_ERR_INVALID_ARG;
+  if (!h->ready) return SPGPE_ERR_NOT_READY;
+  int rc = norms_to(h, h->dout);
+  if (rc) return rc;
+  CK(cudaMemcpyAsync(out, h->dout, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return SPGPE_OK;
+}
+
+extern "C" int spgpe_energy(spgpe_handle h, double out[5]) {
+  if (!h || !out) return SPGPE_ERR_INVALID_ARG;
+  if (!h->ready) return SPGPE_ERR_NOT_READY;
+  if (!h->scratch) CK(cudaMalloc(&h->scratch, h->psi_bytes));
+  const double w = (h->Lx / h->nx) * (h->Ly / h->ny);
+  const int nblk = 1024;
+  h->launches += 4;
+  CK(aux_energy_partials(h->dt, h->psi, h->V, h->Om, h->De, h->points, h->p.g_uu, h->p.g_dd, h->p.g_ud,
+                         h->partial, nblk, h->stream));
+  CK(aux_sum_partials(h->partial, nblk, 3, w, h->dout + 2, h->stream));
+  PassXArgs xa;
+  memset(&xa, 0, sizeof(xa));
+  xa.src = h->psi; xa.dst = h->scratch; xa.tw = h->tw_x;
+  CK(dispatch_x(h, MODE_FWD, xa));
+  PassYArgs ya;
+  memset(&ya, 0, sizeof(ya));
+  ya.psi = h->scratch; ya.tw = h->tw_y; ya.Kx = h->Kx; ya.Ky = h->Ky; ya.partial = h->partial; ya.nx = h->nx;
+  CK(dispatch_y(h, YMODE_ENERGY, ya));
+  CK(aux_sum_partials(h->partial, h->nx / plan_lines(h->ny), 1, w / ((double)h->nx * (double)h->ny), h->dout + 1,
+                      h->stream));
+  double tmp[5];
+  CK(cudaMemcpyAsync(tmp + 1, h->dout + 1, 4 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  out[1] = tmp[1]; out[2] = tmp[2]; out[3] = tmp[3]; out[4] = tmp[4];
+  out[0] = out[1] + out[2] + out[3] + out[4];
+  return SPGPE_OK;
+}
+
+extern "C" int spgpe_synchronize(spgpe_handle h) {
+  if (!h) return SPGPE_ERR_INVALID_ARG;
+  CK(cudaStreamSynchronize(h->stream));
+  return SPGPE_OK;
+}
+extern "C" long long spgpe_launch_count(spgpe_handle h) { return h ? h->launches : -1; }
+
+extern "C" const char* spgpe_strerror(int code) {
+  switch (code) {
+    case SPGPE_OK: return "ok";
+    case SPGPE_ERR_INVALID_ARG: return "invalid argument";
+    case SPGPE_ERR_UNSUPPORTED: return "unsupported grid size (nx, ny must be powers of two in [64, 4096])";
+    case SPGPE_ERR_NOT_READY: return "no order parameter set (call spgpe_set_psi first)";
+    case SPGPE_ERR_CUDA: return "CUDA error (see spgpe_last_cuda_error)";
+    case SPGPE_ERR_NO_DEVICE: return "no sm_100 CUDA device";
+    default: return "unknown error code";
+  }
+}
+extern "C" const char* spgpe_last_cuda_error(void) { return g_cuda_err; }
+
+extern "C" int spgpe_probe_dfma(void* cuda_stream, double* tflops) {
+  if (!tflops) return SPGPE_ERR_INVALID_ARG;
+  CK(aux_probe_dfma((cudaStream_t)cuda_stream, tflops));
+  return SPGPE_OK;
+}
+extern "C" int spgpe_probe_copy(void* cuda_stream, long long bytes, double* gbs) {
+  if (!gbs || bytes <= 0) return SPGPE_ERR_INVALID_ARG;
+  CK(aux_probe_copy((cudaStream_t)cuda_stream, bytes, gbs));
+  return SPGPE_OK;
+}

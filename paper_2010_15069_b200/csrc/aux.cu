@@ -1,0 +1,247 @@
+// aux.cu -- the small kernels around the two pass kernels: k-space phase tables, norm / energy
+// reductions (fixed summation order, fp64 accumulation), imaginary-time rescale, peak probes.
+#include "internal.h"
+
+namespace spgpe {
+
+// ---- k-space phase tables (Eq. 5, R-1..R-3) ---------------------------------------
+// exk[c][pos] = exp(-i Kx_c dt) (imag: exp(-Kx_c dt)); eyk[pos] = exp(-i Ky dt) / (nx ny) (imag: exp(-Ky dt)/(nx ny))
+__global__ void phase_tables_kernel(const double* __restrict__ Kx, const double* __restrict__ Ky, int nx, int ny,
+                                    double dt, int imag, double2* exk, double2* eyk) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int total = 2 * nx + ny;
+  if (i >= total) return;
+  const bool is_y = i >= 2 * nx;
+  const double K = is_y ? Ky[i - 2 * nx] : Kx[i];
+  const double s = is_y ? 1.0 / ((double)nx * (double)ny) : 1.0;
+  double2 r;
+  if (imag) {
+    r = make_double2(s * exp(-K * dt), 0.0);
+  } else {
+    double sn, cn;
+    sincos(K * dt, &sn, &cn);
+    r = make_double2(s * cn, -s * sn);
+  }
+  if (is_y) eyk[i - 2 * nx] = r;
+  else exk[i] = r;
+}
+
+cudaError_t aux_phase_tables(const double* Kx, const double* Ky, int nx, int ny, double dt, int imag,
+                             double2* exk, double2* eyk, cudaStream_t s) {
+  const int total = 2 * nx + ny;
+  phase_tables_kernel<<<(total + 255) / 256, 256, 0, s>>>(Kx, Ky, nx, ny, dt, imag, exk, eyk);
+  return cudaGetLastError();
+}
+
+// ---- deterministic block reduction helper ---------------------------------------------------------------------
+template <int NV>
+__device__ __forceinline__ void block_reduce(double (&x)[NV], double* out_or_null, double (*red)[32]) {
+#pragma unroll
+  for (int v = 0; v < NV; ++v)
+#pragma unroll
+    for (int m = 16; m >= 1; m >>= 1) x[v] += __shfl_xor_sync(0xffffffffu, x[v], m);
+  const int w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  if ((threadIdx.x & 31) == 0)
+    for (int v = 0; v < NV; ++v) red[v][w] = x[v];
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int v = 0; v < NV; ++v) {
+      double s = 0.0;
+      for (int i = 0; i < nw; ++i) s += red[v][i];
+      out_or_null[v] = s;
+    }
+  }
+}
+
+// out[col] = factor * sum_blk partial[blk][col]; one CTA, fixed order
+__global__ void sum_partials_kernel(const double* __restrict__ partial, int nblk, int ncol, double factor,
+                                    double* out) {
+  __shared__ double red[1][32];
+  for (int col = 0; col < ncol; ++col) {
+    double x[1] = {0.0};
+    for (int b = threadIdx.x; b < nblk; b += blockDim.x) x[0] += partial[(size_t)b * ncol + col];
+    double r[1];
+    block_reduce<1>(x, r, red);
+    if (threadIdx.x == 0) out[col] = factor * r[0];
+    __syncthreads();
+  }
+}
+cudaError_t aux_sum_partials(const double* partial, int nblk, int ncol, double factor, double* out,
+                             cudaStream_t s) {
+  sum_partials_kernel<<<1, 256, 0, s>>>(partial, nblk, ncol, factor, out);
+  return cudaGetLastError();
+}
+
+// imaginary-time renormalisation factors (R-7)
+__global__ void norm_scale_kernel(const double* __restrict__ partial, int nblk, double w,
+                                  const double* __restrict__ target, int norm_mode, double* scale) {
+  __shared__ double red[2][32];
+  double x[2] = {0.0, 0.0};
+  for (int b = threadIdx.x; b < nblk; b += blockDim.x) {
+    x[0] += partial[2 * (size_t)b];
+    x[1] += partial[2 * (size_t)b + 1];
+  }
+  double r[2];
+  block_reduce<2>(x, r, red);
+  if (threadIdx.x == 0) {
+    const double nu = w * r[0], nd = w * r[1];
+    if (norm_mode == 0) {
+      scale[0] = sqrt(target[0] / nu);
+      scale[1] = sqrt(target[1] / nd);
+    } else {
+      scale[0] = scale[1] = sqrt((target[0] + target[1]) / (nu + nd));
+    }
+  }
+}
+cudaError_t aux_norm_scale(const double* partial, int nblk, double w, const double* target, int norm_mode,
+                           double* scale, cudaStream_t s) {
+  norm_scale_kernel<<<1, 256, 0, s>>>(partial, nblk, w, target, norm_mode, scale);
+  return cudaGetLastError();
+}
+
+template <int DT>
+__global__ void apply_scale_kernel(void* psi, size_t points, const double* __restrict__ scale) {
+  const double s0 = scale[0], s1 = scale[1];
+  const size_t n = points * 2;  // complex elements
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    cplx z = Store<DT>::ld(psi, i);
+    const double s = (i & 1) ? s1 : s0;
+    Store<DT>::st(psi, i, mk(z.re * s, z.im * s));
+  }
+}
+cudaError_t aux_apply_scale(int dt, void* psi, size_t points, const double* scale, cudaStream_t s) {
+  const int blocks = (int)((points * 2 + 255) / 256 < 148 * 8 ? (points * 2 + 255) / 256 : 148 * 8);
+  if (dt == 0) apply_scale_kernel<0><<<blocks, 256, 0, s>>>(psi, points, scale);
+  else apply_scale_kernel<1><<<blocks, 256, 0, s>>>(psi, points, scale);
+  return cudaGetLastError();
+}
+
+template <int DT>
+__global__ void norm_partials_kernel(const void* __restrict__ psi, size_t points, double* partial) {
+  __shared__ double red[2][32];
+  double x[2] = {0.0, 0.0};
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < points; i += (size_t)gridDim.x * blockDim.x) {
+    cplx u = Store<DT>::ld(psi, 2 * i), d = Store<DT>::ld(psi, 2 * i + 1);
+    x[0] += fma(u.re, u.re, u.im * u.im);
+    x[1] += fma(d.re, d.re, d.im * d.im);
+  }
+  block_reduce<2>(x, partial + 2 * (size_t)blockIdx.x, red);
+}
+cudaError_t aux_norm_partials(int dt, const void* psi, size_t points, double* partial, int nblk, cudaStream_t s) {
+  if (dt == 0) norm_partials_kernel<0><<<nblk, 256, 0, s>>>(psi, points, partial);
+  else norm_partials_kernel<1><<<nblk, 256, 0, s>>>(psi, points, partial);
+  return cudaGetLastError();
+}
+
+// real-space energy terms (R-8): V (n_up + n_dn) + (delta/2)(n_up - n_dn); (g_uu/2) n_up^2 + (g_dd/2) n_dn^2 +
+// g_ud n_up n_dn; Omega Re(conj(psi_up) psi_dn)
+template <int DT>
+__global__ void energy_partials_kernel(const void* __restrict__ psi, const void* __restrict__ V,
+                                       const void* __restrict__ Om, const void* __restrict__ De, size_t points,
+                                       double g_uu, double g_dd, double g_ud, double* partial) {
+  __shared__ double red[3][32];
+  double x[3] = {0.0, 0.0, 0.0};
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < points; i += (size_t)gridDim.x * blockDim.x) {
+    cplx u = Store<DT>::ld(psi, 2 * i), d = Store<DT>::ld(psi, 2 * i + 1);
+    const double nu = fma(u.re, u.re, u.im * u.im), nd = fma(d.re, d.re, d.im * d.im);
+    const double v = V ? Store<DT>::ldr(V, i) : 0.0;
+    const double om = Om ? Store<DT>::ldr(Om, i) : 0.0;
+    const double de = De ? Store<DT>::ldr(De, i) : 0.0;
+    x[0] += v * (nu + nd) + 0.5 * de * (nu - nd);
+    x[1] += 0.5 * g_uu * nu * nu + 0.5 * g_dd * nd * nd + g_ud * nu * nd;
+    x[2] += om * (u.re * d.re + u.im * d.im);
+  }
+  block_reduce<3>(x, partial + 3 * (size_t)blockIdx.x, red);
+}
+cudaError_t aux_energy_partials(int dt, const void* psi, const void* V, const void* Om, const void* De,
+                                size_t points, double g_uu, double g_dd, double g_ud, double* partial, int nblk,
+                                cudaStream_t s) {
+  if (dt == 0)
+    energy_partials_kernel<0><<<nblk, 256, 0, s>>>(psi, V, Om, De, points, g_uu, g_dd, g_ud, partial);
+  else
+    energy_partials_kernel<1><<<nblk, 256, 0, s>>>(psi, V, Om, De, points, g_uu, g_dd, g_ud, partial);
+  return cudaGetLastError();
+}
+
+__global__ void set_targets_kernel(double* target, double a, double b) {
+  target[0] = a;
+  target[1] = b;
+}
+cudaError_t aux_set_targets(double* target, double n_up, double n_dn, cudaStream_t s) {
+  set_targets_kernel<<<1, 1, 0, s>>>(target, n_up, n_dn);
+  return cudaGetLastError();
+}
+
+// ---- peak probes ---------------------------------------------------------------------------------------------
+__global__ void dfma_probe_kernel(double* out, int iters) {
+  double a0 = threadIdx.x * 1e-9, a1 = a0 + 1.0, a2 = a0 + 2.0, a3 = a0 + 3.0;
+  double a4 = a0 + 4.0, a5 = a0 + 5.0, a6 = a0 + 6.0, a7 = a0 + 7.0;
+  const double m = 0.999999, b = 1e-7;
+  for (int i = 0; i < iters; ++i) {
+    a0 = fma(a0, m, b); a1 = fma(a1, m, b); a2 = fma(a2, m, b); a3 = fma(a3, m, b);
+    a4 = fma(a4, m, b); a5 = fma(a5, m, b); a6 = fma(a6, m, b); a7 = fma(a7, m, b);
+  }
+  if (a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7 == 123.456) out[0] = a0;
+}
+cudaError_t aux_probe_dfma(cudaStream_t s, double* tflops) {
+  double* d = nullptr;
+  cudaError_t e = cudaMalloc(&d, 8);
+  if (e != cudaSuccess) return e;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  const int blocks = 148 * 4, threads = 512, iters = 1 << 16;
+  dfma_probe_kernel<<<blocks, threads, 0, s>>>(d, iters / 16);  // warm-up
+  float best = 1e30f;
+  for (int r = 0; r < 3; ++r) {
+    cudaEventRecord(e0, s);
+    dfma_probe_kernel<<<blocks, threads, 0, s>>>(d, iters);
+    cudaEventRecord(e1, s);
+    e = cudaEventSynchronize(e1);
+    if (e != cudaSuccess) break;
+    float ms;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (ms < best) best = ms;
+  }
+  *tflops = 2.0 * 8.0 * (double)iters * blocks * threads / (best * 1e-3) * 1e-12;
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(d);
+  return e;
+}
+
+__global__ void copy_probe_kernel(const double2* __restrict__ src, double2* __restrict__ dst, size_t n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    dst[i] = src[i];
+}
+cudaError_t aux_probe_copy(cudaStream_t s, long long bytes, double* gbs) {
+  char *a = nullptr, *b = nullptr;
+  cudaError_t e = cudaMalloc(&a, bytes);
+  if (e != cudaSuccess) return e;
+  e = cudaMalloc(&b, bytes);
+  if (e != cudaSuccess) { cudaFree(a); return e; }
+  cudaMemsetAsync(a, 1, bytes, s);
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0);
+  cudaEventCreate(&e1);
+  const size_t n = (size_t)bytes / sizeof(double2);
+  float best = 1e30f;
+  for (int r = 0; r < 6; ++r) {
+    cudaEventRecord(e0, s);
+    copy_probe_kernel<<<148 * 16, 512, 0, s>>>((const double2*)a, (double2*)b, n);
+    cudaEventRecord(e1, s);
+    e = cudaEventSynchronize(e1);
+    if (e != cudaSuccess) break;
+    float ms;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (r > 0 && ms < best) best = ms;
+  }
+  *gbs = 2.0 * (double)bytes / (best * 1e-3) * 1e-9;
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(a);
+  cudaFree(b);
+  return e;
+}
+
+}  // namespace spgpe

@@ -1,0 +1,104 @@
+// common.cuh -- complex arithmetic in registers, storage-precision loads/stores, plan constants.
+// Part of libspgpe (CUDA path).  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace spgpe {
+
+struct cplx {
+  double re, im;
+};
+
+__device__ __forceinline__ cplx mk(double r, double i) { cplx c; c.re = r; c.im = i; return c; }
+__device__ __forceinline__ cplx operator+(cplx a, cplx b) { return mk(a.re + b.re, a.im + b.im); }
+__device__ __forceinline__ cplx operator-(cplx a, cplx b) { return mk(a.re - b.re, a.im - b.im); }
+// a * b
+__device__ __forceinline__ cplx cmul(cplx a, cplx b) {
+  return mk(fma(a.re, b.re, -(a.im * b.im)), fma(a.re, b.im, a.im * b.re));
+}
+// a * conj(b)
+__device__ __forceinline__ cplx cmulc(cplx a, cplx b) {
+  return mk(fma(a.re, b.re, a.im * b.im), fma(a.im, b.re, -(a.re * b.im)));
+}
+// multiply by +i (D=+1) or -i (D=-1)
+template <int D>
+__device__ __forceinline__ cplx mul_i(cplx a) {
+  return D > 0 ? mk(-a.im, a.re) : mk(a.im, -a.re);
+}
+
+// ---- storage precision: C128 = double2 per component, C64 = float2 per component -----------------
+template <int DT> struct Store;
+template <> struct Store<0> {
+  typedef double real;
+  typedef double2 elem;
+  static __device__ __forceinline__ cplx ld(const void* base, size_t idx) {
+    double2 v = reinterpret_cast<const double2*>(base)[idx];
+    return mk(v.x, v.y);
+  }
+  static __device__ __forceinline__ void st(void* base, size_t idx, cplx c) {
+    reinterpret_cast<double2*>(base)[idx] = make_double2(c.re, c.im);
+  }
+  static __device__ __forceinline__ double ldr(const void* base, size_t idx) {
+    return __ldg(reinterpret_cast<const double*>(base) + idx);
+  }
+};
+template <> struct Store<1> {
+  typedef float real;
+  typedef float2 elem;
+  static __device__ __forceinline__ cplx ld(const void* base, size_t idx) {
+    float2 v = reinterpret_cast<const float2*>(base)[idx];
+    return mk((double)v.x, (double)v.y);
+  }
+  static __device__ __forceinline__ void st(void* base, size_t idx, cplx c) {
+    reinterpret_cast<float2*>(base)[idx] = make_float2((float)c.re, (float)c.im);
+  }
+  static __device__ __forceinline__ double ldr(const void* base, size_t idx) {
+    return (double)__ldg(reinterpret_cast<const float*>(base) + idx);
+  }
+};
+
+// ---- transform plan: N = 16 * 16 * ... * R_LAST, every thread holds 16 points of one component ----
+// Stage j (1-based) has radix 16 and stride M_j = N / 16^j; the last stage has radix R_LAST and the
+// thread runs G = 16 / R_LAST butterflies on groups q = t + g*T of R_LAST consecutive positions.
+template <int N> struct Plan;
+#define SPGPE_PLAN(N_, NS_, RL_)                                             \
+  template <> struct Plan<N_> {                                              \
+    static constexpr int NS = NS_;     /* number of stages */               \
+    static constexpr int RL = RL_;     /* radix of the last stage */        \
+    static constexpr int T = N_ / 16;  /* threads per component per line */ \
+    static constexpr int G = 16 / RL_; /* groups per thread, last stage */  \
+    static constexpr int PADSHIFT = (RL_ == 16 ? 4 : RL_ == 4 ? 2 : 3);      \
+    static constexpr int PTS = N_ + (N_ >> PADSHIFT); /* padded points */    \
+  };
+SPGPE_PLAN(64, 2, 4)
+SPGPE_PLAN(128, 2, 8)
+SPGPE_PLAN(256, 2, 16)
+SPGPE_PLAN(512, 3, 2)
+SPGPE_PLAN(1024, 3, 4)
+SPGPE_PLAN(2048, 3, 8)
+SPGPE_PLAN(4096, 3, 16)
+#undef SPGPE_PLAN
+
+// stride of radix-16 stage j (1-based, j < NS)
+template <int N>
+__host__ __device__ constexpr int stage_stride(int j) {
+  int m = N;
+  for (int i = 0; i < j; ++i) m /= 16;
+  return m;
+}
+
+// offset of stage j's twiddle block in the per-N twiddle table: block j holds 15 * M_j entries,
+// entry (k-1) * M_j + lo = exp(-2 pi i k lo / (16 M_j)), k = 1..15
+template <int N>
+__host__ __device__ constexpr int tw_offset(int j) {
+  int off = 0;
+  for (int i = 1; i < j; ++i) off += 15 * stage_stride<N>(i);
+  return off;
+}
+template <int N>
+__host__ __device__ constexpr int tw_total() {
+  return tw_offset<N>(Plan<N>::NS);
+}
+
+}  // namespace spgpe

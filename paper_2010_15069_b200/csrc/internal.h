@@ -1,0 +1,51 @@
+// internal.h -- declarations shared by the translation units of libspgpe (host side).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "pass_x.cuh"
+#include "pass_y.cuh"
+
+namespace spgpe {
+
+// per-length launchers (inst_<N>.cu)
+#define SPGPE_DECL(N_)                                                                          \
+  cudaError_t launch_pass_x_##N_(int dt, int mode, const PassXArgs& a, int ny, cudaStream_t s); \
+  cudaError_t launch_pass_y_##N_(int dt, int ymode, const PassYArgs& a, cudaStream_t s);
+SPGPE_DECL(64)
+SPGPE_DECL(128)
+SPGPE_DECL(256)
+SPGPE_DECL(512)
+SPGPE_DECL(1024)
+SPGPE_DECL(2048)
+SPGPE_DECL(4096)
+#undef SPGPE_DECL
+
+// host-side plan queries (tables.cu)
+int plan_tw_total(int n);                       // number of twiddle entries of length n
+void plan_fill_twiddles(int n, double2* host);  // exp(-2 pi i k lo / (16 M_j)) blocks, see common.cuh
+int plan_freq_of_pos(int n, int pos);           // signed-less frequency index f in [0, n) stored at position pos
+int plan_lines(int n);                          // lines per CTA of the pass kernels of length n
+
+// small kernels (aux.cu); all enqueue on s and return cudaGetLastError()
+cudaError_t aux_phase_tables(const double* Kx, const double* Ky, int nx, int ny, double dt, int imag,
+                             double2* exk, double2* eyk, cudaStream_t s);
+// partial[nblk][ncol] -> out[col] = factor * sum_blk partial[blk][col]   (fixed summation order)
+cudaError_t aux_sum_partials(const double* partial, int nblk, int ncol, double factor, double* out,
+                             cudaStream_t s);
+// scale[c] = sqrt(target[c] / (w * sum_blk partial[blk][c]))  (per component) or common factor (total)
+cudaError_t aux_norm_scale(const double* partial, int nblk, double w, const double* target, int norm_mode,
+                           double* scale, cudaStream_t s);
+cudaError_t aux_apply_scale(int dt, void* psi, size_t points, const double* scale, cudaStream_t s);
+// partial[nblk][2]: sum |psi_c|^2 ; returns nblk used through *nblk (<= max_blk)
+cudaError_t aux_norm_partials(int dt, const void* psi, size_t points, double* partial, int nblk,
+                              cudaStream_t s);
+// partial[nblk][3]: potential+Zeeman, interaction, Raman sums (without dx dy)
+cudaError_t aux_energy_partials(int dt, const void* psi, const void* V, const void* Om, const void* De,
+                                size_t points, double g_uu, double g_dd, double g_ud, double* partial,
+                                int nblk, cudaStream_t s);
+cudaError_t aux_set_targets(double* target, double n_up, double n_dn, cudaStream_t s);
+// probes (bench roofline denominators)
+cudaError_t aux_probe_dfma(cudaStream_t s, double* tflops);
+cudaError_t aux_probe_copy(cudaStream_t s, long long bytes, double* gbs);
+
+}  // namespace spgpe

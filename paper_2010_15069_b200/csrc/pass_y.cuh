@@ -1,0 +1,92 @@
+// pass_y.cuh -- the column pass: y-direction forward transform, k-space phase, inverse transform
+// (SURVEY.md 8(a) rows a2/a4 (y part) and a3; include/spgpe.h).  The k-space factor
+// exp(-i K_c dt) is separable: the k_x factor is applied at the end of the row pass, here only
+// ey(k_y) = exp(-i k_y^2 dt / 2) / (nx ny) (imaginary time: the decaying real factor).
+//
+// One CTA handles LINES adjacent columns; thread index = c + 2*(line + LINES*t), so that a warp-wide access
+// covers LINES*32 contiguous bytes in each of 16/LINES rows.
+//
+//   YMODE_STEP   : psi^(k_x, y) -> F_y -> * ey(k_y) -> F_y^-1 -> psi^(k_x, y)            (in place)
+//   YMODE_ENERGY : psi^(k_x, y) -> F_y -> sum (Kx_c(k_x) + Ky(k_y)) |psi^|^2 -> partial[CTA]
+#pragma once
+#include "line_fft.cuh"
+
+namespace spgpe {
+
+enum { YMODE_STEP = 0, YMODE_ENERGY = 1 };
+
+struct PassYArgs {
+  void* psi;            // [NY][nx][2]
+  const double2* tw;    // twiddles of NY
+  const double2* eyk;   // [NY] k_y phase in stored order (YMODE_STEP)
+  const double* Kx;     // [2][nx] (k_x +- k_L)^2/2 in the row pass's stored order (YMODE_ENERGY)
+  const double* Ky;     // [NY] k_y^2/2 in stored order (YMODE_ENERGY)
+  double* partial;      // [gridDim.x] (YMODE_ENERGY)
+  int nx;
+};
+
+template <int NY, int LINES>
+struct YLayout {
+  // padded points per line buffer; the residue mod 4 keeps a quarter-warp's lines on distinct banks
+  static constexpr int BASE = Plan<NY>::PTS;
+  static constexpr int WANT = (LINES >= 4) ? 1 : (LINES == 2 ? 2 : 0);
+  static constexpr int LINE_PTS = BASE + ((WANT - (BASE & 3)) & 3);
+};
+
+template <int DT, int NY, int LINES, int YMODE>
+__global__ void __launch_bounds__(LINES * (NY / 8), (LINES * (NY / 8) <= 256) ? 2 : 1)
+pass_y_kernel(const PassYArgs a) {
+  typedef Plan<NY> P;
+  typedef Store<DT> St;
+  extern __shared__ double2 smem[];
+  constexpr int T = P::T;
+  const int tid = threadIdx.x;
+  const int c = tid & 1;
+  const int line = (tid >> 1) % LINES;
+  const int t = (tid >> 1) / LINES;
+  double2* buf = smem + (size_t)line * (YLayout<NY, LINES>::LINE_PTS * 2);
+  const size_t col = (size_t)blockIdx.x * LINES + line;
+  const size_t nx = (size_t)a.nx;
+  cplx v[16];
+
+#pragma unroll
+  for (int n = 0; n < 16; ++n) v[n] = St::ld(a.psi, ((size_t)(t + n * T) * nx + col) * 2 + c);
+
+  line_fft_fwd<NY>(buf, a.tw, t, c, v);
+
+  if (YMODE == YMODE_STEP) {
+#pragma unroll
+    for (int g = 0; g < P::G; ++g)
+#pragma unroll
+      for (int s = 0; s < P::RL; ++s) {
+        double2 e = __ldg(a.eyk + (t + g * T) + (NY / P::RL) * s);
+        v[g * P::RL + s] = cmul(v[g * P::RL + s], mk(e.x, e.y));
+      }
+    line_fft_inv<NY>(buf, a.tw, t, c, v);
+#pragma unroll
+    for (int n = 0; n < 16; ++n) St::st(a.psi, ((size_t)(t + n * T) * nx + col) * 2 + c, v[n]);
+  } else {
+    const double kx = a.Kx[(size_t)c * nx + col];
+    double e = 0.0;
+#pragma unroll
+    for (int g = 0; g < P::G; ++g)
+#pragma unroll
+      for (int s = 0; s < P::RL; ++s) {
+        const cplx z = v[g * P::RL + s];
+        e = fma(kx + a.Ky[(t + g * T) + (NY / P::RL) * s], fma(z.re, z.re, z.im * z.im), e);
+      }
+    __shared__ double red[32];
+#pragma unroll
+    for (int m = 16; m >= 1; m >>= 1) e += __shfl_xor_sync(0xffffffffu, e, m);
+    const int w = tid >> 5, nw = (blockDim.x + 31) >> 5;
+    if ((tid & 31) == 0) red[w] = e;
+    __syncthreads();
+    if (tid == 0) {
+      double s0 = 0.0;
+      for (int i = 0; i < nw; ++i) s0 += red[i];
+      a.partial[blockIdx.x] = s0;
+    }
+  }
+}
+
+}  // namespace spgpe

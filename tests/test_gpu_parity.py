@@ -1,0 +1,196 @@
+"""Parity of the CUDA path (through the C ABI of include/spgpe.h) with the CPU oracle, element by element,
+on the same seeded inputs.  Tolerances are BASELINE.json's: relative L2 of psi <= 1e-10 (complex128),
+<= 1e-4 (complex64 storage); energy within 1e-9 relative (complex128).
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle as orc
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL_C128 = 1e-10
+TOL_C64 = 1e-4
+TOL_E = 1e-9
+
+
+@pytest.fixture(scope="module")
+def sp():
+    import torch
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    import paper_2010_15069_b200 as sp_
+    sp_.lib()  # fails loudly if libspgpe.so is missing
+    return sp_
+
+
+def rel_l2(a, b):
+    return np.linalg.norm((a.astype(np.complex128) - b).ravel()) / np.linalg.norm(b.ravel())
+
+
+def random_problem(nx, ny, seed, g=(1.0, 0.8, 0.6), k_L=0.7):
+    r = np.random.default_rng(seed)
+    Lx, Ly = 12.0, 10.0
+    x = wl.configs.grid(nx, Lx)
+    y = wl.configs.grid(ny, Ly)
+    X, Y = np.meshgrid(x, y)
+    psi = (np.exp(-0.3 * (X * X + Y * Y))[:, :, None] * (1.0 + 0.3 * r.standard_normal((ny, nx, 2))) *
+           np.exp(1j * (0.5 * X + 0.2 * r.standard_normal((ny, nx))))[:, :, None])
+    psi = np.ascontiguousarray(psi.astype(np.complex128))
+    V = 0.5 * (X * X + 0.8 * Y * Y) + 0.1 * r.standard_normal((ny, nx))
+    Om = 1.5 * np.tanh(Y) + 0.2
+    De = 0.3 * X + 0.1
+    p = orc.params(nx, ny, Lx, Ly, g[0], g[1], g[2], k_L, 0)
+    return psi, V, Om, De, p, (Lx, Ly)
+
+
+def make_solver(sp, psi, V, Om, De, p, dtype="c128"):
+    dt = sp.SPGPE_C128 if dtype == "c128" else sp.SPGPE_C64
+    h = sp.spgpe_create(p.nx, p.ny, p.Lx, p.Ly, dt, p.g_uu, p.g_dd, p.g_ud, p.k_L, p.norm_mode)
+    cdt, rdt = h._np_dtypes
+    sp.spgpe_set_potential(h, None if V is None else np.ascontiguousarray(V, dtype=rdt))
+    sp.spgpe_set_raman(h, None if Om is None else np.ascontiguousarray(Om, dtype=rdt))
+    sp.spgpe_set_zeeman(h, None if De is None else np.ascontiguousarray(De, dtype=rdt))
+    sp.spgpe_set_psi_host(h, np.ascontiguousarray(psi, dtype=cdt))
+    return h
+
+
+SIZES = [(64, 64), (128, 64), (64, 256), (256, 128), (512, 64), (64, 1024), (1024, 128), (128, 2048),
+         (2048, 64), (4096, 64), (64, 4096)]
+
+
+@pytest.mark.parametrize("nx,ny", SIZES)
+def test_real_time_steps_match_oracle(sp, nx, ny):
+    """Every supported line length in x and in y (each spans its own radix plan), non-square grids."""
+    psi, V, Om, De, p, _ = random_problem(nx, ny, seed=nx * 7 + ny)
+    h = make_solver(sp, psi, V, Om, De, p)
+    n, dt = 3, 2e-3
+    sp.spgpe_step(h, n, dt, 0)
+    got = sp.spgpe_get_psi_host(h)
+    ref = orc.step(psi, V, Om, De, p, n, dt, 0)
+    assert rel_l2(got, ref) < TOL_C128
+    # step(n) then step(m) equals step(n+m)
+    sp.spgpe_step(h, 2, dt, 0)
+    ref2 = orc.step(ref, V, Om, De, p, 2, dt, 0)
+    assert rel_l2(sp.spgpe_get_psi_host(h), ref2) < TOL_C128
+
+
+@pytest.mark.parametrize("nx,ny", [(64, 64), (256, 128), (128, 512), (1024, 64)])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_imaginary_time_steps_match_oracle(sp, nx, ny, mode):
+    psi, V, Om, De, p, _ = random_problem(nx, ny, seed=5 + nx + ny)
+    p.norm_mode = mode
+    h = make_solver(sp, psi, V, Om, De, p)
+    n, dt = 4, 1e-3
+    sp.spgpe_step(h, n, dt, 1)
+    got = sp.spgpe_get_psi_host(h)
+    ref = orc.step(psi, V, Om, De, p, n, dt, 1)
+    assert rel_l2(got, ref) < TOL_C128
+    np.testing.assert_allclose(sp.spgpe_norm(h), orc.norm(ref, p), rtol=1e-12)
+
+
+@pytest.mark.parametrize("nx,ny", [(64, 64), (256, 64), (128, 1024), (2048, 128)])
+def test_norm_and_energy_match_oracle(sp, nx, ny):
+    psi, V, Om, De, p, _ = random_problem(nx, ny, seed=99 + nx)
+    h = make_solver(sp, psi, V, Om, De, p)
+    np.testing.assert_allclose(sp.spgpe_norm(h), orc.norm(psi, p), rtol=1e-13)
+    e_ref = orc.energy(psi, V, Om, De, p)
+    e_got = sp.spgpe_energy(h)
+    scale = np.abs(e_ref).max()
+    assert np.abs(e_got - e_ref).max() < TOL_E * scale, (e_got, e_ref)
+    # energy does not disturb the state
+    assert rel_l2(sp.spgpe_get_psi_host(h), psi) == 0.0
+
+
+def test_null_fields_and_zero_coupling(sp):
+    """NULL fields mean zero; Omega = 0, g = 0 reduces to free evolution + nothing else."""
+    psi, V, Om, De, p, _ = random_problem(128, 128, seed=3, g=(0.0, 0.0, 0.0), k_L=0.0)
+    h = make_solver(sp, psi, None, None, None, p)
+    sp.spgpe_step(h, 5, 1e-3, 0)
+    ref = orc.step(psi, None, None, None, p, 5, 1e-3, 0)
+    assert rel_l2(sp.spgpe_get_psi_host(h), ref) < TOL_C128
+
+
+def test_negative_dt_and_large_arguments(sp):
+    """dt < 0 works; large V*tau and |b|*tau leave the series' range and take the libm branch."""
+    psi, V, Om, De, p, _ = random_problem(128, 64, seed=17)
+    V = 300.0 * V
+    Om = 400.0 * Om
+    h = make_solver(sp, psi, V, Om, De, p)
+    sp.spgpe_step(h, 2, -5e-3, 0)
+    ref = orc.step(psi, V, Om, De, p, 2, -5e-3, 0)
+    assert rel_l2(sp.spgpe_get_psi_host(h), ref) < TOL_C128
+    h2 = make_solver(sp, psi, V * 0.05, Om * 0.3, De, p)
+    sp.spgpe_step(h2, 2, 5e-3, 1)
+    ref2 = orc.step(psi, V * 0.05, Om * 0.3, De, p, 2, 5e-3, 1)
+    assert rel_l2(sp.spgpe_get_psi_host(h2), ref2) < TOL_C128
+
+
+def test_device_tensor_interface_and_stream(sp):
+    """Device-pointer entry points with torch tensors on a non-default stream."""
+    import torch
+    psi, V, Om, De, p, _ = random_problem(256, 256, seed=21)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        h = sp.spgpe_create(p.nx, p.ny, p.Lx, p.Ly, sp.SPGPE_C128, p.g_uu, p.g_dd, p.g_ud, p.k_L, 0,
+                            stream=st.cuda_stream)
+        dV, dO, dD = (torch.from_numpy(a).cuda() for a in (V, Om, De))
+        dpsi = torch.from_numpy(psi).cuda()
+        st.synchronize()
+        sp.spgpe_set_potential(h, dV)
+        sp.spgpe_set_raman(h, dO)
+        sp.spgpe_set_zeeman(h, dD)
+        sp.spgpe_set_psi(h, dpsi)
+        sp.spgpe_step(h, 4, 1e-3, 0)
+        out = torch.empty_like(dpsi)
+        sp.spgpe_get_psi(h, out)
+        sp.spgpe_synchronize(h)
+    ref = orc.step(psi, V, Om, De, p, 4, 1e-3, 0)
+    assert rel_l2(out.cpu().numpy(), ref) < TOL_C128
+
+
+def test_error_codes(sp):
+    with pytest.raises(sp.SpgpeError) as e:
+        sp.spgpe_create(100, 64, 1.0, 1.0)
+    assert e.value.code == -2
+    with pytest.raises(sp.SpgpeError) as e:
+        sp.spgpe_create(64, 64, -1.0, 1.0)
+    assert e.value.code == -1
+    h = sp.spgpe_create(64, 64, 1.0, 1.0)
+    with pytest.raises(sp.SpgpeError) as e:
+        sp.spgpe_step(h, 1, 1e-3, 0)
+    assert e.value.code == -3
+
+
+@pytest.mark.parametrize("nx,ny", [(256, 256), (1024, 64)])
+def test_c64_storage_matches_oracle(sp, nx, ny):
+    psi, V, Om, De, p, _ = random_problem(nx, ny, seed=31)
+    # inputs rounded to fp32 first; those values go to both sides (reading R-14)
+    psi = psi.astype(np.complex64).astype(np.complex128)
+    V, Om, De = (a.astype(np.float32).astype(np.float64) for a in (V, Om, De))
+    h = make_solver(sp, psi, V, Om, De, p, dtype="c64")
+    sp.spgpe_step(h, 20, 1e-3, 0)
+    ref = orc.step(psi, V, Om, De, p, 20, 1e-3, 0)
+    assert rel_l2(sp.spgpe_get_psi_host(h), ref) < TOL_C64
+
+
+# ---- the five workloads of BASELINE.json (proxy sizes the oracle finishes in seconds; full sizes below) ----
+@pytest.mark.parametrize("cfg,n,steps", [(1, 64, None), (2, 256, 100), (3, 256, 100), (4, 256, 100), (5, 256, 50)])
+def test_workload_configs_proxy(sp, cfg, n, steps):
+    dtype = "c64" if cfg == 5 else "c128"
+    w = wl.make_workload(cfg, n=n, dtype=dtype)
+    h = sp.from_workload(w)
+    p = orc.params_of(w)
+    ref = w.psi0
+    for (cnt, dt, imag) in w.schedule:
+        cnt = cnt if steps is None else min(cnt, steps)
+        sp.spgpe_step(h, cnt, dt, imag)
+        ref = orc.step(ref, w.V, w.Omega, w.delta, p, cnt, dt, imag)
+    got = sp.spgpe_get_psi_host(h)
+    assert rel_l2(got, ref) < (TOL_C64 if dtype == "c64" else TOL_C128)
+    if dtype == "c128":
+        e_ref = orc.energy(ref, w.V, w.Omega, w.delta, p)
+        e_got = sp.spgpe_energy(h)
+        assert np.abs(e_got - e_ref).max() < TOL_E * np.abs(e_ref).max()
