@@ -1,0 +1,324 @@
+#!/usr/bin/env python
+"""bench.py -- split-step throughput of libspgpe on BASELINE.json's metric workload (config 4: 2048 x 2048,
+two components, complex128, real time, dt = 2.5e-4), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload 4|4c64|3|2|1]
+
+A "step" is one Strang step of the whole hot path (a6 in imaginary time).
+  value      : grid-point-steps/s (P = nx*ny counted once, not per component) over all N replicas, state and
+               fields resident in HBM, CUDA events around ONE spgpe_step(K) call, max over ranks.
+  e2e        : the same metric through the C ABI with HOST buffers: set_potential/raman/zeeman_host +
+               set_psi_host (pinned) -> spgpe_step(K) -> get_psi_host, copies inside the timed region (the
+               paper's usage: order parameter in, M steps, order parameter out).
+  roofline   : dominant kernel (the longer of the row pass and the column pass), timed per launch with CUDA
+               events on the handle's stream (spgpe_profile) over a second region of K steps.
+  cpu_baseline: the oracle as it stands, on this box's host cores, a bounded sample of the same workload.
+Multi-GPU: replicas only: every rank steps its own copy of the workload, no collective
+on the data path; value = N * P * K / max-over-ranks time.
+--impl reference times the oracle (oracle/) on the host cores; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "split-step grid-point-steps/s"
+UNIT = "grid-point-steps/s"
+# algorithmic bytes per grid point per launch: psi read + written once per
+# pass; the row pass also reads the fields in use (one real per point each)
+WORKLOADS = {
+    "4": dict(cfg=4, dtype="c128"), "4c64": dict(cfg=4, dtype="c64"), "3": dict(cfg=3, dtype="c128"),
+    "2": dict(cfg=2, dtype="c128"), "1": dict(cfg=1, dtype="c128"),
+}
+
+
+def read_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """SM clock and throttle reasons sampled through NVML while the timed regions run."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz, self.ok = [], set(), None, False
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.dev = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.dev, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:  # NVML missing: report that, do not fail the bench
+            self.err = repr(e)
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4),
+            "hw_power_brake": getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80),
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.dev, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.dev))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.dev))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.005)
+
+    def start(self):
+        if self.ok:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        if self._thr:
+            self._stop.set()
+            self._thr.join()
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "note": "NVML unavailable"}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def oracle_sample(w_cfg: int, dtype: str, budget_s: float, steps: int):
+    """Times the oracle on a proxy grid of the same recipe, chosen so that `steps` steps fit the budget.
+    Returns (grid-point-steps/s, threads, description, seconds per step)."""
+    import oracle as orc
+    import workloads as wl
+    threads = orc.max_threads()
+    full = wl.CONFIGS[w_cfg]["n"]
+    n, sec = 64, None
+    while True:
+        w = wl.make_workload(w_cfg, n=n, dtype=dtype)
+        p = orc.params_of(w)
+        cnt, dt, imag = w.schedule[0]
+        t0 = time.perf_counter()
+        orc.step(w.psi0, w.V, w.Omega, w.delta, p, 1, dt, imag)
+        sec = time.perf_counter() - t0
+        if n >= full or 4.2 * sec * steps > budget_s:  # the next size costs ~4.2x
+            break
+        n *= 2
+    t0 = time.perf_counter()
+    orc.step(w.psi0, w.V, w.Omega, w.delta, p, steps, dt, imag)
+    sec = (time.perf_counter() - t0) / steps
+    what = (f"{steps} oracle steps (fp64, own radix-2 FFT, OpenMP) of config {w_cfg}'s recipe on a {n}x{n} "
+            f"grid (full size {full}x{full}), {'imaginary' if imag else 'real'} time")
+    return n * n / sec, threads, what, sec
+
+
+def run_reference(args, wname):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    spec = WORKLOADS[wname]
+    import oracle as orc
+    import workloads as wl
+    threads = orc.max_threads()
+    full = wl.CONFIGS[spec["cfg"]]["n"]
+    total = args.steps + args.warmup
+    # pick the largest proxy grid whose whole run fits ~150 s
+    n = 64
+    while n < full:
+        w = wl.make_workload(spec["cfg"], n=n, dtype=spec["dtype"])
+        p = orc.params_of(w)
+        cnt, dt, imag = w.schedule[0]
+        t0 = time.perf_counter()
+        orc.step(w.psi0, w.V, w.Omega, w.delta, p, 1, dt, imag)
+        sec = time.perf_counter() - t0
+        if 4.2 * sec * total > 150.0:
+            break
+        n *= 2
+    w = wl.make_workload(spec["cfg"], n=n, dtype=spec["dtype"])
+    p = orc.params_of(w)
+    cnt, dt, imag = w.schedule[0]
+    psi = orc.step(w.psi0, w.V, w.Omega, w.delta, p, args.warmup, dt, imag)
+    t0 = time.perf_counter()
+    orc.step(psi, w.V, w.Omega, w.delta, p, args.steps, dt, imag)
+    el = time.perf_counter() - t0
+    value = n * n * args.steps / el
+    sample = (f"each step = one oracle Strang step of config {spec['cfg']}'s recipe on a {n}x{n} proxy grid "
+              f"(full size {full}x{full}); fp64, own radix-2 FFT, OpenMP over lines")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"config {spec['cfg']} recipe, {n}x{n} proxy of {full}x{full}, "
+                               f"{spec['dtype']} inputs, oracle on host cores"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, wname):
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libspgpe has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import paper_2010_15069_b200 as sp
+    import workloads as wl
+    sp.lib()  # fails loudly when libspgpe.so is missing
+
+    spec = WORKLOADS[wname]
+    w = wl.make_workload(spec["cfg"], dtype=spec["dtype"])
+    cnt, dt, imag = w.schedule[0]
+    K, W = args.steps, args.warmup
+    P = w.points
+    stream = torch.cuda.Stream()
+    h = sp.from_workload(w, stream=stream.cuda_stream)
+    cdt, rdt = h._np_dtypes
+    esz = np.dtype(cdt).itemsize
+    rsz = np.dtype(rdt).itemsize
+    nfields = sum(f is not None for f in (w.V, w.Omega, w.delta))
+    psi_bytes = 2 * P * esz
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed_region(fn):
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            fn()
+            e1.record(stream)
+        barrier()
+        ms = torch.tensor([e0.elapsed_time(e1)], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+        return float(ms.item())
+
+    sampler = ClockSampler(local)
+    # ---- device-resident throughput --------------------------------------------------------------------
+    sp.spgpe_step(h, W, dt, imag)
+    sp.spgpe_synchronize(h)
+    sampler.start()
+    l0 = sp.spgpe_launch_count(h)
+    ms = timed_region(lambda: sp.spgpe_step(h, K, dt, imag))
+    launches = sp.spgpe_launch_count(h) - l0
+    # ---- per-launch durations of the two pass kernels (second region of K steps) -----------------------
+    sp.spgpe_profile(h, True)
+    sp.spgpe_step(h, K, dt, imag)
+    kms, kcnt = sp.spgpe_profile_read(h)
+    sp.spgpe_profile(h, False)
+    clocks = sampler.stop()
+    # ---- end to end through the host-buffer calls --------------------------------------------------------
+    pin = torch.from_numpy(np.ascontiguousarray(w.psi0, dtype=cdt)).pin_memory()
+    pout = torch.empty_like(pin).pin_memory()
+    fields = [None if f is None else torch.from_numpy(np.ascontiguousarray(f, dtype=rdt)).pin_memory()
+              for f in (w.V, w.Omega, w.delta)]
+    L = sp.lib()
+
+    def e2e_job():
+        for name, f in zip(("potential", "raman", "zeeman"), fields):
+            sp._check(getattr(L, f"spgpe_set_{name}_host")(h.ptr, None if f is None else f.data_ptr()))
+        sp._check(L.spgpe_set_psi_host(h.ptr, pin.data_ptr()))
+        sp._check(L.spgpe_step(h.ptr, K, dt, imag))
+        sp._check(L.spgpe_get_psi_host(h.ptr, pout.data_ptr()))
+
+    e2e_job()  # warm-up (page-locks, first-touch)
+    barrier()
+    t0 = time.perf_counter()
+    e2e_job()  # ends with a stream synchronise inside get_psi_host
+    barrier()
+    e2e_s = torch.tensor([time.perf_counter() - t0], device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+    e2e_s = float(e2e_s.item())
+    finite = bool(np.isfinite(pout.numpy().view(rdt)).all())
+    norms = sp.spgpe_norm(h)
+
+    if rank == 0:
+        peak, peak_src = read_peaks()
+        # dominant kernel = the pass with the longer average launch
+        avg = [kms[i] / max(1, kcnt[i]) for i in range(2)]
+        dom = 0 if avg[0] >= avg[1] else 1
+        bytes_pt = [2 * 2 * esz + nfields * rsz, 2 * 2 * esz]  # row pass: psi r+w + fields; column pass: psi r+w
+        achieved = bytes_pt[dom] * P / (avg[dom] * 1e-3) / 1e9
+        step_bytes = (bytes_pt[0] + bytes_pt[1]) * P
+        line = {
+            "metric": METRIC, "value": world * P * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
+            "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "grid": [w.nx, w.ny], "storage": spec["dtype"],
+                       "time": "imaginary" if imag else "real", "dt": dt, "parallelism": "replicas only",
+                       "l2": f"state {psi_bytes >> 20} MiB + fields {(nfields * P * rsz) >> 20} MiB per replica; "
+                             + ("larger than the 126 MB L2, no flush" if psi_bytes > 126e6 else
+                                "fits L2: the HBM roofline is not the binding bound")},
+            "steps_per_s": world * K / (ms * 1e-3),
+            "step_hbm_gbs": step_bytes / (ms / K * 1e-3) / 1e9,
+            "step_roofline_frac": step_bytes / (ms / K * 1e-3) / 1e9 / peak,
+            "roofline": {"bound": "hbm", "kernel": ["pass_x_kernel (row pass)", "pass_y_kernel (column pass)"][dom],
+                         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "peak_source": peak_src,
+                         "avg_launch_us": {"row_pass": 1e3 * avg[0], "column_pass": 1e3 * avg[1]},
+                         "launches_timed": kcnt, "bytes_per_point": bytes_pt},
+            "e2e": {"value": world * P * K / e2e_s, "unit": UNIT,
+                    "h2d_bytes_per_step": (psi_bytes + nfields * P * rsz) / K, "d2h_bytes_per_step": psi_bytes / K,
+                    "job": f"fields + psi host->device, spgpe_step({K}), psi device->host; {e2e_s:.4f} s"},
+            "gpu_launches": int(launches), "clocks": clocks, "finite": finite, "norms": list(map(float, norms)),
+        }
+        if world == 1 and not args.no_cpu:
+            v, cores, what, sec = oracle_sample(spec["cfg"], spec["dtype"], budget_s=25.0, steps=3)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what,
+                                    "s_per_step": sec}
+        print(json.dumps(line), flush=True)
+    sp.spgpe_destroy(h)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="4", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args, args.workload)
+    else:
+        run_ours(args, args.workload)
+
+
+if __name__ == "__main__":
+    main()

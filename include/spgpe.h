@@ -97,6 +97,13 @@ int spgpe_energy(spgpe_handle h, double out[5]);
 int spgpe_synchronize(spgpe_handle h);
 /* Number of kernels the handle has launched so far (bench.py's gpu_launches claim). */
 long long spgpe_launch_count(spgpe_handle h);
+/* Per-launch timing with CUDA events on the handle's stream (measurement only; bench.py's roofline).
+ * spgpe_profile(h, 1) synchronises and starts recording an event pair around every row-pass and column-pass
+ * launch of later spgpe_step calls; spgpe_profile_read synchronises, returns the summed durations in
+ * milliseconds and the launch counts per class (0 = row pass, 1 = column pass) and resets the record;
+ * spgpe_profile(h, 0) stops.  Host arrays. */
+int spgpe_profile(spgpe_handle h, int enable);
+int spgpe_profile_read(spgpe_handle h, double h_ms[2], long long h_count[2]);
 const char* spgpe_strerror(int code);
 const char* spgpe_last_cuda_error(void);
 

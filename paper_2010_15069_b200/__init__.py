@@ -29,6 +29,7 @@ ABI_SYMBOLS = (
     "spgpe_set_potential_host", "spgpe_set_raman_host", "spgpe_set_zeeman_host",
     "spgpe_set_psi", "spgpe_get_psi", "spgpe_set_psi_host", "spgpe_get_psi_host", "spgpe_set_norm_targets",
     "spgpe_step", "spgpe_norm", "spgpe_energy", "spgpe_synchronize", "spgpe_launch_count",
+    "spgpe_profile", "spgpe_profile_read",
     "spgpe_strerror", "spgpe_last_cuda_error", "spgpe_probe_dfma", "spgpe_probe_copy",
 )
 
@@ -74,6 +75,8 @@ def lib() -> ctypes.CDLL:
         L.spgpe_energy.argtypes = [vp, ctypes.POINTER(cd)]
         L.spgpe_launch_count.argtypes = [vp]
         L.spgpe_launch_count.restype = ctypes.c_longlong
+        L.spgpe_profile.argtypes = [vp, ci]
+        L.spgpe_profile_read.argtypes = [vp, ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_longlong)]
         L.spgpe_strerror.argtypes = [ci]
         L.spgpe_strerror.restype = ctypes.c_char_p
         L.spgpe_last_cuda_error.restype = ctypes.c_char_p
@@ -224,6 +227,18 @@ def spgpe_synchronize(h: Handle) -> None:
 
 def spgpe_launch_count(h: Handle) -> int:
     return int(lib().spgpe_launch_count(h.ptr))
+
+
+def spgpe_profile(h: Handle, enable: bool) -> None:
+    _check(lib().spgpe_profile(h.ptr, int(bool(enable))))
+
+
+def spgpe_profile_read(h: Handle):
+    """(ms[2], count[2]): summed CUDA-event durations and launch counts of the row pass and the column pass."""
+    ms = (ctypes.c_double * 2)()
+    cnt = (ctypes.c_longlong * 2)()
+    _check(lib().spgpe_profile_read(h.ptr, ms, cnt))
+    return list(ms), list(cnt)
 
 
 def spgpe_probe_dfma(stream: Optional[int] = None) -> float:

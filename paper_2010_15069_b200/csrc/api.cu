@@ -33,7 +33,34 @@ struct spgpe_ctx {
   bool ready;
   long long launches;
   HalfCoef hc;
+  // per-launch CUDA-event timing (spgpe_profile): pairs of events around every row/column pass launch
+  bool prof_on;
+  std::vector<cudaEvent_t>* prof_ev;  // [2*i], [2*i+1] = start, stop of launch i
+  std::vector<int>* prof_cls;         // class of launch i: 0 row pass, 1 column pass
+  size_t prof_used;
 };
+
+static cudaError_t prof_begin(spgpe_ctx* h, int cls) {
+  if (!h->prof_on) return cudaSuccess;
+  if (h->prof_ev->size() < 2 * (h->prof_used + 1)) {
+    cudaEvent_t a, b;
+    cudaError_t e = cudaEventCreate(&a);
+    if (e != cudaSuccess) return e;
+    e = cudaEventCreate(&b);
+    if (e != cudaSuccess) return e;
+    h->prof_ev->push_back(a);
+    h->prof_ev->push_back(b);
+    h->prof_cls->push_back(cls);
+  }
+  (*h->prof_cls)[h->prof_used] = cls;
+  return cudaEventRecord((*h->prof_ev)[2 * h->prof_used], h->stream);
+}
+static cudaError_t prof_end(spgpe_ctx* h) {
+  if (!h->prof_on) return cudaSuccess;
+  cudaError_t e = cudaEventRecord((*h->prof_ev)[2 * h->prof_used + 1], h->stream);
+  h->prof_used++;
+  return e;
+}
 
 static thread_local char g_cuda_err[256] = "";
 
@@ -49,8 +76,7 @@ static int cuda_fail(cudaError_t e) {
 
 static bool size_ok(int n) { return n >= 64 && n <= 4096 && (n & (n - 1)) == 0; }
 
-static cudaError_t dispatch_x(spgpe_ctx* h, int mode, const PassXArgs& a) {
-  h->launches++;
+static cudaError_t dispatch_x_raw(spgpe_ctx* h, int mode, const PassXArgs& a) {
   switch (h->nx) {
     case 64: return launch_pass_x_64(h->dt, mode, a, h->ny, h->stream);
     case 128: return launch_pass_x_128(h->dt, mode, a, h->ny, h->stream);
@@ -61,8 +87,7 @@ static cudaError_t dispatch_x(spgpe_ctx* h, int mode, const PassXArgs& a) {
     default: return launch_pass_x_4096(h->dt, mode, a, h->ny, h->stream);
   }
 }
-static cudaError_t dispatch_y(spgpe_ctx* h, int ymode, const PassYArgs& a) {
-  h->launches++;
+static cudaError_t dispatch_y_raw(spgpe_ctx* h, int ymode, const PassYArgs& a) {
   switch (h->ny) {
     case 64: return launch_pass_y_64(h->dt, ymode, a, h->stream);
     case 128: return launch_pass_y_128(h->dt, ymode, a, h->stream);
@@ -72,6 +97,23 @@ static cudaError_t dispatch_y(spgpe_ctx* h, int ymode, const PassYArgs& a) {
     case 2048: return launch_pass_y_2048(h->dt, ymode, a, h->stream);
     default: return launch_pass_y_4096(h->dt, ymode, a, h->stream);
   }
+}
+
+static cudaError_t dispatch_x(spgpe_ctx* h, int mode, const PassXArgs& a) {
+  h->launches++;
+  cudaError_t e = prof_begin(h, 0);
+  if (e != cudaSuccess) return e;
+  e = dispatch_x_raw(h, mode, a);
+  if (e != cudaSuccess) return e;
+  return prof_end(h);
+}
+static cudaError_t dispatch_y(spgpe_ctx* h, int ymode, const PassYArgs& a) {
+  h->launches++;
+  cudaError_t e = prof_begin(h, 1);
+  if (e != cudaSuccess) return e;
+  e = dispatch_y_raw(h, ymode, a);
+  if (e != cudaSuccess) return e;
+  return prof_end(h);
 }
 
 // kinetic tables in the stored order of the transforms (Eq. 5; R-2, R-3, R-9)
@@ -121,6 +163,8 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
   h->hc.ca_d = 0.5 * (p->g_dd + p->g_ud);
   h->hc.cb_u = 0.5 * (p->g_uu - p->g_ud);
   h->hc.cb_d = 0.5 * (p->g_ud - p->g_dd);
+  h->prof_ev = new std::vector<cudaEvent_t>();
+  h->prof_cls = new std::vector<int>();
   h->partial_cap = 4 * (nx > ny ? nx : ny);
   if (h->partial_cap < 4 * 2048) h->partial_cap = 4 * 2048;
 
@@ -173,6 +217,11 @@ extern "C" int spgpe_destroy(spgpe_handle h) {
                   h->exk, h->eyk, h->partial, h->scale, h->target, h->dout};
   for (void* p : ptrs)
     if (p) cudaFree(p);
+  if (h->prof_ev) {
+    for (cudaEvent_t ev : *h->prof_ev) cudaEventDestroy(ev);
+    delete h->prof_ev;
+    delete h->prof_cls;
+  }
   delete h;
   return SPGPE_OK;
 }
@@ -332,6 +381,28 @@ extern "C" int spgpe_energy(spgpe_handle h, double out[5]) {
 extern "C" int spgpe_synchronize(spgpe_handle h) {
   if (!h) return SPGPE_ERR_INVALID_ARG;
   CK(cudaStreamSynchronize(h->stream));
+  return SPGPE_OK;
+}
+extern "C" int spgpe_profile(spgpe_handle h, int enable) {
+  if (!h) return SPGPE_ERR_INVALID_ARG;
+  CK(cudaStreamSynchronize(h->stream));
+  h->prof_on = enable != 0;
+  h->prof_used = 0;
+  return SPGPE_OK;
+}
+extern "C" int spgpe_profile_read(spgpe_handle h, double ms[2], long long count[2]) {
+  if (!h || !ms || !count) return SPGPE_ERR_INVALID_ARG;
+  CK(cudaStreamSynchronize(h->stream));
+  ms[0] = ms[1] = 0.0;
+  count[0] = count[1] = 0;
+  for (size_t i = 0; i < h->prof_used; ++i) {
+    float t = 0.f;
+    CK(cudaEventElapsedTime(&t, (*h->prof_ev)[2 * i], (*h->prof_ev)[2 * i + 1]));
+    const int c = (*h->prof_cls)[i];
+    ms[c] += (double)t;
+    count[c]++;
+  }
+  h->prof_used = 0;
   return SPGPE_OK;
 }
 extern "C" long long spgpe_launch_count(spgpe_handle h) { return h ? h->launches : -1; }
