@@ -27,6 +27,12 @@ __device__ __forceinline__ cplx mul_i(cplx a) {
   return D > 0 ? mk(-a.im, a.re) : mk(a.im, -a.re);
 }
 
+// A zero that the compiler cannot see through: g_zero is a __constant__ 0, so (bits of x) & g_zero is 0 but
+// carries a data dependency on x.  Added to the index of a table load it pins the load after the producer
+// of x; without it ptxas hoists all twiddle / phase-table loads to the top of the kernel and spills.
+static __constant__ int g_zero = 0;
+__device__ __forceinline__ int late_zero(double x) { return __double2hiint(x) & g_zero; }
+
 // ---- storage precision: C128 = double2 per component, C64 = float2 per component -----------------
 template <int DT> struct Store;
 template <> struct Store<0> {

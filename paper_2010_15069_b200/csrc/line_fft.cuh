@@ -73,7 +73,8 @@ __device__ __forceinline__ void twiddle(const double2* __restrict__ tw, int t, c
   const double2* w = tw + tw_offset<N>(J) + lo;
 #pragma unroll
   for (int k = 1; k < 16; ++k) {
-    double2 d = __ldg(w + (k - 1) * M);
+    // the address depends on v[k] (late_zero), so that ptxas cannot hoist the table load far above its use
+    double2 d = __ldg(w + (k - 1) * M + late_zero(v[k].re));
     v[k] = (D < 0) ? cmul(v[k], mk(d.x, d.y)) : cmulc(v[k], mk(d.x, d.y));
   }
 }

@@ -44,6 +44,12 @@ __device__ __forceinline__ void real_space(cplx* v, const PassXArgs& a, size_t r
                                            double& su, double& sd) {
   typedef Store<DT> St;
   constexpr int T = NX / 16;
+  // fields of the thread's 8 points, fetched one point ahead of their use (the loads of point i+1 are in
+  // flight while point i is being evaluated)
+  const size_t x0 = rowbase + t + (8 * c) * T;
+  double Vn = a.V ? St::ldr(a.V, x0) : 0.0;
+  double On = a.Om ? St::ldr(a.Om, x0) : 0.0;
+  double Dn = a.De ? St::ldr(a.De, x0) : 0.0;
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     // send what the partner needs, receive the partner's component at my points
@@ -52,10 +58,13 @@ __device__ __forceinline__ void real_space(cplx* v, const PassXArgs& a, size_t r
     cplx recv = shfl_xor_c(send, 1);
     cplx up = c ? recv : mine;
     cplx dn = c ? mine : recv;
-    const size_t x = rowbase + t + (i + 8 * c) * T;
-    const double Vv = a.V ? St::ldr(a.V, x) : 0.0;
-    const double Ov = a.Om ? St::ldr(a.Om, x) : 0.0;
-    const double Dv = a.De ? St::ldr(a.De, x) : 0.0;
+    const double Vv = Vn, Ov = On, Dv = Dn;
+    if (i < 7) {
+      const size_t x = x0 + (i + 1) * T;
+      Vn = a.V ? St::ldr(a.V, x) : 0.0;
+      On = a.Om ? St::ldr(a.Om, x) : 0.0;
+      Dn = a.De ? St::ldr(a.De, x) : 0.0;
+    }
     if (MODE == MODE_MID) {
       double a1 = su2_apply<false>(up, dn, Vv, Ov, Dv, a.tau, a.hc);
       double a2 = su2_apply<false>(up, dn, Vv, Ov, Dv, a.tau, a.hc);
@@ -151,7 +160,7 @@ pass_x_kernel(const PassXArgs a) {
         const int pos = (t + g * T) + (NX / P::RL) * s;
         cplx o = v[g * P::RL + s];
         if (MODE != MODE_FWD) {
-          double2 e = __ldg(a.exk + c * NX + pos);
+          double2 e = __ldg(a.exk + c * NX + pos + late_zero(o.re));
           o = cmul(o, mk(e.x, e.y));
         }
         St::st(a.dst, (rowbase + pos) * 2 + c, o);

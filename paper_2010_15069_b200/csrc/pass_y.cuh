@@ -49,8 +49,11 @@ pass_y_kernel(const PassYArgs a) {
   const size_t nx = (size_t)a.nx;
   cplx v[16];
 
+  // element (row t, column col, component c); rows of one thread are T*nx points apart
+  const size_t e0 = ((size_t)t * nx + col) * 2 + c;
+  const size_t estride = (size_t)T * nx * 2;
 #pragma unroll
-  for (int n = 0; n < 16; ++n) v[n] = St::ld(a.psi, ((size_t)(t + n * T) * nx + col) * 2 + c);
+  for (int n = 0; n < 16; ++n) v[n] = St::ld(a.psi, e0 + n * estride);
 
   line_fft_fwd<NY>(buf, a.tw, t, c, v);
 
@@ -59,12 +62,15 @@ pass_y_kernel(const PassYArgs a) {
     for (int g = 0; g < P::G; ++g)
 #pragma unroll
       for (int s = 0; s < P::RL; ++s) {
-        double2 e = __ldg(a.eyk + (t + g * T) + (NY / P::RL) * s);
+        double2 e = __ldg(a.eyk + (t + g * T) + (NY / P::RL) * s + late_zero(v[g * P::RL + s].re));
         v[g * P::RL + s] = cmul(v[g * P::RL + s], mk(e.x, e.y));
       }
     line_fft_inv<NY>(buf, a.tw, t, c, v);
+    // recompute the addresses instead of keeping 16 of them alive across both transforms
+    size_t e1 = e0;
+    asm volatile("" : "+l"(e1));
 #pragma unroll
-    for (int n = 0; n < 16; ++n) St::st(a.psi, ((size_t)(t + n * T) * nx + col) * 2 + c, v[n]);
+    for (int n = 0; n < 16; ++n) St::st(a.psi, e1 + n * estride, v[n]);
   } else {
     const double kx = a.Kx[(size_t)c * nx + col];
     double e = 0.0;
