@@ -32,6 +32,7 @@ struct spgpe_ctx {
   int partial_cap;
   bool ready;
   long long launches;
+  int xgrid;  // CTAs of the last row-pass launch (rows of `partial` it wrote)
   HalfCoef hc;
   // per-launch CUDA-event timing (spgpe_profile): pairs of events around every row/column pass launch
   bool prof_on;
@@ -78,13 +79,13 @@ static bool size_ok(int n) { return n >= 64 && n <= 4096 && (n & (n - 1)) == 0; 
 
 static cudaError_t dispatch_x_raw(spgpe_ctx* h, int mode, const PassXArgs& a) {
   switch (h->nx) {
-    case 64: return launch_pass_x_64(h->dt, mode, a, h->ny, h->stream);
-    case 128: return launch_pass_x_128(h->dt, mode, a, h->ny, h->stream);
-    case 256: return launch_pass_x_256(h->dt, mode, a, h->ny, h->stream);
-    case 512: return launch_pass_x_512(h->dt, mode, a, h->ny, h->stream);
-    case 1024: return launch_pass_x_1024(h->dt, mode, a, h->ny, h->stream);
-    case 2048: return launch_pass_x_2048(h->dt, mode, a, h->ny, h->stream);
-    default: return launch_pass_x_4096(h->dt, mode, a, h->ny, h->stream);
+    case 64: return launch_pass_x_64(h->dt, mode, a, h->ny, h->stream, &h->xgrid);
+    case 128: return launch_pass_x_128(h->dt, mode, a, h->ny, h->stream, &h->xgrid);
+    case 256: return launch_pass_x_256(h->dt, mode, a, h->ny, h->stream, &h->xgrid);
+    case 512: return launch_pass_x_512(h->dt, mode, a, h->ny, h->stream, &h->xgrid);
+    case 1024: return launch_pass_x_1024(h->dt, mode, a, h->ny, h->stream, &h->xgrid);
+    case 2048: return launch_pass_x_2048(h->dt, mode, a, h->ny, h->stream, &h->xgrid);
+    default: return launch_pass_x_4096(h->dt, mode, a, h->ny, h->stream, &h->xgrid);
   }
 }
 static cudaError_t dispatch_y_raw(spgpe_ctx* h, int ymode, const PassYArgs& a) {
@@ -313,11 +314,10 @@ extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
   memset(&xa, 0, sizeof(xa));
   xa.src = h->psi; xa.dst = h->psi; xa.V = h->V; xa.Om = h->Om; xa.De = h->De;
   xa.tw = h->tw_x; xa.exk = h->exk; xa.scale = nullptr; xa.partial = h->partial;
-  xa.tau = 0.5 * dt; xa.hc = h->hc; xa.imag = imag; xa.want_norm = imag;
+  xa.tau = 0.5 * dt; xa.hc = h->hc; xa.imag = imag; xa.want_norm = imag; xa.ny = h->ny;
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
   ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx;
-  const int xblocks = h->ny / plan_lines(h->nx);
   const double w = (h->Lx / h->nx) * (h->Ly / h->ny);
   if (!imag) {
     CK(dispatch_x(h, MODE_PRO, xa));
@@ -332,7 +332,7 @@ extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
       CK(dispatch_y(h, YMODE_STEP, ya));
       CK(dispatch_x(h, MODE_EPI, xa));
       h->launches++;
-      CK(aux_norm_scale(h->partial, xblocks, w, h->target, h->p.norm_mode, h->scale, h->stream));
+      CK(aux_norm_scale(h->partial, h->xgrid, w, h->target, h->p.norm_mode, h->scale, h->stream));
     }
     h->launches++;
     CK(aux_apply_scale(h->dt, h->psi, h->points, h->scale, h->stream));
@@ -362,13 +362,13 @@ extern "C" int spgpe_energy(spgpe_handle h, double out[5]) {
   CK(aux_sum_partials(h->partial, nblk, 3, w, h->dout + 2, h->stream));
   PassXArgs xa;
   memset(&xa, 0, sizeof(xa));
-  xa.src = h->psi; xa.dst = h->scratch; xa.tw = h->tw_x;
+  xa.src = h->psi; xa.dst = h->scratch; xa.tw = h->tw_x; xa.ny = h->ny;
   CK(dispatch_x(h, MODE_FWD, xa));
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
   ya.psi = h->scratch; ya.tw = h->tw_y; ya.Kx = h->Kx; ya.Ky = h->Ky; ya.partial = h->partial; ya.nx = h->nx;
   CK(dispatch_y(h, YMODE_ENERGY, ya));
-  CK(aux_sum_partials(h->partial, h->nx / plan_lines(h->ny), 1, w / ((double)h->nx * (double)h->ny), h->dout + 1,
+  CK(aux_sum_partials(h->partial, h->nx / plan_lines_y(h->ny), 1, w / ((double)h->nx * (double)h->ny), h->dout + 1,
                       h->stream));
   double tmp[5];
   CK(cudaMemcpyAsync(tmp + 1, h->dout + 1, 4 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));

@@ -34,12 +34,25 @@ static __constant__ int g_zero = 0;
 __device__ __forceinline__ int late_zero(double x) { return __double2hiint(x) & g_zero; }
 
 // ---- storage precision: C128 = double2 per component, C64 = float2 per component -----------------
+// psi streams through the kernels once per pass: its loads bypass L1 allocation (L1::no_allocate) so that the
+// twiddle and phase tables, which every thread re-reads, stay resident there.
+__device__ __forceinline__ double2 ldg_stream(const double2* p) {
+  double2 v;
+  asm volatile("ld.global.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ float2 ldg_stream(const float2* p) {
+  float2 v;
+  asm volatile("ld.global.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+  return v;
+}
+
 template <int DT> struct Store;
 template <> struct Store<0> {
   typedef double real;
   typedef double2 elem;
   static __device__ __forceinline__ cplx ld(const void* base, size_t idx) {
-    double2 v = reinterpret_cast<const double2*>(base)[idx];
+    double2 v = ldg_stream(reinterpret_cast<const double2*>(base) + idx);
     return mk(v.x, v.y);
   }
   static __device__ __forceinline__ void st(void* base, size_t idx, cplx c) {
@@ -48,12 +61,15 @@ template <> struct Store<0> {
   static __device__ __forceinline__ double ldr(const void* base, size_t idx) {
     return __ldg(reinterpret_cast<const double*>(base) + idx);
   }
+  static __device__ __forceinline__ double lds(const void* base, int idx) {
+    return reinterpret_cast<const double*>(base)[idx];
+  }
 };
 template <> struct Store<1> {
   typedef float real;
   typedef float2 elem;
   static __device__ __forceinline__ cplx ld(const void* base, size_t idx) {
-    float2 v = reinterpret_cast<const float2*>(base)[idx];
+    float2 v = ldg_stream(reinterpret_cast<const float2*>(base) + idx);
     return mk((double)v.x, (double)v.y);
   }
   static __device__ __forceinline__ void st(void* base, size_t idx, cplx c) {
@@ -62,7 +78,22 @@ template <> struct Store<1> {
   static __device__ __forceinline__ double ldr(const void* base, size_t idx) {
     return (double)__ldg(reinterpret_cast<const float*>(base) + idx);
   }
+  static __device__ __forceinline__ double lds(const void* base, int idx) {
+    return (double)reinterpret_cast<const float*>(base)[idx];
+  }
 };
+
+// ---- asynchronous copies ------------------------------------------------------------------------------------
+// 16-byte global -> shared copy that bypasses registers (LDGSTS); completion through cp_async_wait_all
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+// ask L2 to fetch `bytes` (multiple of 16) starting at the 16-byte aligned address p; no registers, no scoreboard
+__device__ __forceinline__ void prefetch_l2_bulk(const void* p, unsigned bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
 
 // ---- transform plan: N = 16 * 16 * ... * R_LAST, every thread holds 16 points of one component ----
 // Stage j (1-based) has radix 16 and stride M_j = N / 16^j; the last stage has radix R_LAST and the

@@ -9,7 +9,7 @@ namespace spgpe {
 
 // per-length launchers (inst_<N>.cu)
 #define SPGPE_DECL(N_)                                                                          \
-  cudaError_t launch_pass_x_##N_(int dt, int mode, const PassXArgs& a, int ny, cudaStream_t s); \
+  cudaError_t launch_pass_x_##N_(int dt, int mode, const PassXArgs& a, int ny, cudaStream_t s, int* grid); \
   cudaError_t launch_pass_y_##N_(int dt, int ymode, const PassYArgs& a, cudaStream_t s);
 SPGPE_DECL(64)
 SPGPE_DECL(128)
@@ -24,7 +24,7 @@ SPGPE_DECL(4096)
 int plan_tw_total(int n);                       // number of twiddle entries of length n
 void plan_fill_twiddles(int n, double2* host);  // exp(-2 pi i k lo / (16 M_j)) blocks, see common.cuh
 int plan_freq_of_pos(int n, int pos);           // signed-less frequency index f in [0, n) stored at position pos
-int plan_lines(int n);                          // lines per CTA of the pass kernels of length n
+int plan_lines_y(int n);                        // columns per CTA of the column pass of length n
 
 // small kernels (aux.cu); all enqueue on s and return cudaGetLastError()
 cudaError_t aux_phase_tables(const double* Kx, const double* Ky, int nx, int ny, double dt, int imag,

@@ -7,20 +7,42 @@
 namespace spgpe {
 
 // lines (rows or columns) per CTA: 256 threads per CTA up to N = 2048, 512 at N = 4096
-template <int N> struct Lines { static constexpr int X = (N >= 2048) ? 1 : (N == 1024 ? 2 : 4), Y = X; };
+template <int N> struct Lines {
+  static constexpr int X = (N >= 2048) ? 1 : (N == 1024 ? 2 : 4);
+  static constexpr int Y = (N >= 4096) ? 1 : (N >= 1024 ? 2 : 4);
+};
 
+// number of CTAs that can be resident on the device at once (persistent row pass)
+template <typename K>
+cudaError_t resident_ctas(K kernel, int threads, size_t smem, int* out) {
+  int dev = 0, sms = 0, occ = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess) return e;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem);
+  if (e != cudaSuccess) return e;
+  *out = sms * (occ > 0 ? occ : 1);
+  return cudaSuccess;
+}
+
+// grid_out: number of CTAs launched (= rows of PassXArgs::partial written by MODE_EPI)
 template <int DT, int N, int MODE>
-cudaError_t launch_x(const PassXArgs& a, int ny, cudaStream_t s) {
+cudaError_t launch_x(const PassXArgs& a, int ny, cudaStream_t s, int* grid_out) {
   constexpr int L = Lines<N>::X;
   auto k = pass_x_kernel<DT, N, L, MODE>;
   constexpr size_t smem = (size_t)L * Plan<N>::PTS * 2 * sizeof(double2);
-  static bool attr_set = false;
-  if (!attr_set) {
+  static int resident = 0;
+  if (resident == 0) {
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    attr_set = true;
+    e = resident_ctas(k, L * (N / 8), smem, &resident);
+    if (e != cudaSuccess) return e;
   }
-  k<<<ny / L, L * (N / 8), smem, s>>>(a);
+  const int groups = ny / L;
+  const int grid = groups < resident ? groups : resident;
+  *grid_out = grid;
+  k<<<grid, L * (N / 8), smem, s>>>(a);
   return cudaGetLastError();
 }
 
@@ -40,20 +62,20 @@ cudaError_t launch_y(const PassYArgs& a, cudaStream_t s) {
 }
 
 #define SPGPE_DEFINE_LAUNCHERS(N_)                                                               \
-  cudaError_t launch_pass_x_##N_(int dt, int mode, const PassXArgs& a, int ny, cudaStream_t s) { \
+  cudaError_t launch_pass_x_##N_(int dt, int mode, const PassXArgs& a, int ny, cudaStream_t s, int* g) { \
     if (dt == 0) {                                                                               \
       switch (mode) {                                                                            \
-        case MODE_PRO: return launch_x<0, N_, MODE_PRO>(a, ny, s);                               \
-        case MODE_MID: return launch_x<0, N_, MODE_MID>(a, ny, s);                               \
-        case MODE_EPI: return launch_x<0, N_, MODE_EPI>(a, ny, s);                               \
-        default: return launch_x<0, N_, MODE_FWD>(a, ny, s);                                     \
+        case MODE_PRO: return launch_x<0, N_, MODE_PRO>(a, ny, s, g);                               \
+        case MODE_MID: return launch_x<0, N_, MODE_MID>(a, ny, s, g);                               \
+        case MODE_EPI: return launch_x<0, N_, MODE_EPI>(a, ny, s, g);                               \
+        default: return launch_x<0, N_, MODE_FWD>(a, ny, s, g);                                     \
       }                                                                                          \
     }                                                                                            \
     switch (mode) {                                                                              \
-      case MODE_PRO: return launch_x<1, N_, MODE_PRO>(a, ny, s);                                 \
-      case MODE_MID: return launch_x<1, N_, MODE_MID>(a, ny, s);                                 \
-      case MODE_EPI: return launch_x<1, N_, MODE_EPI>(a, ny, s);                                 \
-      default: return launch_x<1, N_, MODE_FWD>(a, ny, s);                                       \
+      case MODE_PRO: return launch_x<1, N_, MODE_PRO>(a, ny, s, g);                                 \
+      case MODE_MID: return launch_x<1, N_, MODE_MID>(a, ny, s, g);                                 \
+      case MODE_EPI: return launch_x<1, N_, MODE_EPI>(a, ny, s, g);                                 \
+      default: return launch_x<1, N_, MODE_FWD>(a, ny, s, g);                                       \
     }                                                                                            \
   }                                                                                              \
   cudaError_t launch_pass_y_##N_(int dt, int ymode, const PassYArgs& a, cudaStream_t s) {        \

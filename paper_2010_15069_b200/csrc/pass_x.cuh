@@ -27,29 +27,53 @@ struct PassXArgs {
   const double2* tw;     // twiddles of NX
   const double2* exk;    // [2][NX] k_x phase in stored order (MODE_PRO, MODE_MID)
   const double* scale;   // [2] per-component factor applied at load (MODE_PRO, imaginary time) or NULL
-  double* partial;       // [gridDim.x][2] sum |psi_c|^2 of this CTA (MODE_EPI with want_norm)
+  double* partial;       // [gridDim.x][2] sum |psi_c|^2 over this CTA's rows (MODE_EPI with want_norm)
   double tau;            // half-step size dt/2
   HalfCoef hc;
   int imag;
   int want_norm;
+  int ny;                // number of rows
 };
 
 __device__ __forceinline__ double shfl_xor_d(double x, int m) { return __shfl_xor_sync(0xffffffffu, x, m); }
 __device__ __forceinline__ cplx shfl_xor_c(cplx a, int m) { return mk(shfl_xor_d(a.re, m), shfl_xor_d(a.im, m)); }
 
+// Copy the three field rows of this CTA's LINES rows into shared memory ([field][line][x], working precision),
+// 16 bytes per cp.async; a NULL field is filled with zeros.  Every thread of the CTA takes part.
+template <int DT, int NX, int LINES>
+__device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, size_t first_point, int tid) {
+  typedef typename Store<DT>::real real;
+  constexpr int FIELD_BYTES = LINES * NX * (int)sizeof(real);
+  constexpr int NCH = FIELD_BYTES / 16;
+  constexpr int NTHR = LINES * (NX / 8);
+  const void* src[3] = {a.V, a.Om, a.De};
+#pragma unroll
+  for (int f = 0; f < 3; ++f) {
+    char* dst = reinterpret_cast<char*>(fbuf) + f * FIELD_BYTES;
+    if (src[f] != nullptr) {
+      const char* g = reinterpret_cast<const char*>(src[f]) + first_point * sizeof(real);
+#pragma unroll
+      for (int k = tid; k < NCH; k += NTHR) cp_async16(dst + k * 16, g + k * 16);
+    } else {
+#pragma unroll
+      for (int k = tid; k < NCH; k += NTHR) *reinterpret_cast<float4*>(dst + k * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+  }
+}
+
 // Real-space part on the thread's registers v[n] = psi_c(x = t + n*T).  Pair exchange: the c=0 thread takes both
-// components of the points n = 0..7, the c=1 thread those of n = 8..15.
-template <int DT, int NX, int MODE>
-__device__ __forceinline__ void real_space(cplx* v, const PassXArgs& a, size_t rowbase, int t, int c,
+// components of the points n = 0..7, the c=1 thread those of n = 8..15.  Fields come from shared memory
+// (stage_fields), index lx = line*NX + x.
+template <int DT, int NX, int LINES, int MODE>
+__device__ __forceinline__ void real_space(cplx* v, const PassXArgs& a, const void* fbuf, int line, int t, int c,
                                            double& su, double& sd) {
   typedef Store<DT> St;
+  typedef typename St::real real;
   constexpr int T = NX / 16;
-  // fields of the thread's 8 points, fetched one point ahead of their use (the loads of point i+1 are in
-  // flight while point i is being evaluated)
-  const size_t x0 = rowbase + t + (8 * c) * T;
-  double Vn = a.V ? St::ldr(a.V, x0) : 0.0;
-  double On = a.Om ? St::ldr(a.Om, x0) : 0.0;
-  double Dn = a.De ? St::ldr(a.De, x0) : 0.0;
+  const real* fV = reinterpret_cast<const real*>(fbuf);
+  const real* fO = fV + LINES * NX;
+  const real* fD = fO + LINES * NX;
+  const double tau = a.tau, tau2 = a.tau * a.tau;
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     // send what the partner needs, receive the partner's component at my points
@@ -58,28 +82,25 @@ __device__ __forceinline__ void real_space(cplx* v, const PassXArgs& a, size_t r
     cplx recv = shfl_xor_c(send, 1);
     cplx up = c ? recv : mine;
     cplx dn = c ? mine : recv;
-    const double Vv = Vn, Ov = On, Dv = Dn;
-    if (i < 7) {
-      const size_t x = x0 + (i + 1) * T;
-      Vn = a.V ? St::ldr(a.V, x) : 0.0;
-      On = a.Om ? St::ldr(a.Om, x) : 0.0;
-      Dn = a.De ? St::ldr(a.De, x) : 0.0;
-    }
+    const int lx = line * NX + t + (i + 8 * c) * T;
+    const double Vv = St::lds(fV, lx);
+    const double hO = 0.5 * St::lds(fO, lx);
+    const double hD = 0.5 * St::lds(fD, lx);
     if (MODE == MODE_MID) {
-      double a1 = su2_apply<false>(up, dn, Vv, Ov, Dv, a.tau, a.hc);
-      double a2 = su2_apply<false>(up, dn, Vv, Ov, Dv, a.tau, a.hc);
+      double a1 = su2_apply<false>(up, dn, Vv, hO, hD, tau, tau2, a.hc);
+      double a2 = su2_apply<false>(up, dn, Vv, hO, hD, tau, tau2, a.hc);
       double pr, pi;
-      phase_eval((a1 + a2) * a.tau, pr, pi);
+      phase_eval((a1 + a2) * tau, pr, pi);
       apply_phase(up, dn, pr, pi);
     } else if (a.imag) {
-      double a1 = su2_apply<true>(up, dn, Vv, Ov, Dv, a.tau, a.hc);
-      double e = exp(-a1 * a.tau);
+      double a1 = su2_apply<true>(up, dn, Vv, hO, hD, tau, tau2, a.hc);
+      double e = exp(-a1 * tau);
       up = mk(up.re * e, up.im * e);
       dn = mk(dn.re * e, dn.im * e);
     } else {
-      double a1 = su2_apply<false>(up, dn, Vv, Ov, Dv, a.tau, a.hc);
+      double a1 = su2_apply<false>(up, dn, Vv, hO, hD, tau, tau2, a.hc);
       double pr, pi;
-      phase_eval(a1 * a.tau, pr, pi);
+      phase_eval(a1 * tau, pr, pi);
       apply_phase(up, dn, pr, pi);
     }
     if (MODE == MODE_EPI) {
@@ -94,11 +115,14 @@ __device__ __forceinline__ void real_space(cplx* v, const PassXArgs& a, size_t r
   }
 }
 
+// Persistent: CTA b handles the row groups b, b + gridDim.x, ...; while one group is being transformed the next
+// one (psi rows and field rows) is requested into L2, so that its loads find the data there.
 template <int DT, int NX, int LINES, int MODE>
 __global__ void __launch_bounds__(LINES * (NX / 8), (LINES * (NX / 8) <= 256) ? 2 : 1)
 pass_x_kernel(const PassXArgs a) {
   typedef Plan<NX> P;
   typedef Store<DT> St;
+  typedef typename St::real real;
   extern __shared__ double2 smem[];
   constexpr int T = P::T;
   const int tid = threadIdx.x;
@@ -106,65 +130,89 @@ pass_x_kernel(const PassXArgs a) {
   const int t = (tid >> 1) % T;
   const int line = (tid >> 1) / T;
   double2* buf = smem + (size_t)line * (P::PTS * 2);
-  const size_t row = (size_t)blockIdx.x * LINES + line;
-  const size_t rowbase = row * NX;  // in points
+  const int ngroups = a.ny / LINES;
+  double su = 0.0, sd = 0.0;
   cplx v[16];
 
-  if (MODE == MODE_PRO || MODE == MODE_FWD) {
-#pragma unroll
-    for (int n = 0; n < 16; ++n) v[n] = St::ld(a.src, (rowbase + t + n * T) * 2 + c);
-    if (MODE == MODE_PRO && a.scale != nullptr) {
-      const double s = a.scale[c];
-#pragma unroll
-      for (int n = 0; n < 16; ++n) v[n] = mk(v[n].re * s, v[n].im * s);
+  for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+    const size_t first_point = (size_t)grp * LINES * NX;  // first point of the CTA's rows
+    const size_t rowbase = first_point + (size_t)line * NX;
+    if (tid == 0 && grp + (int)gridDim.x < ngroups) {
+      const size_t nxt = (size_t)(grp + gridDim.x) * LINES * NX;
+      prefetch_l2_bulk(reinterpret_cast<const typename St::elem*>(a.src) + nxt * 2,
+                       LINES * NX * 2 * (unsigned)sizeof(typename St::elem));
+      if (MODE != MODE_FWD) {
+        if (a.V) prefetch_l2_bulk(reinterpret_cast<const real*>(a.V) + nxt, LINES * NX * (unsigned)sizeof(real));
+        if (a.Om) prefetch_l2_bulk(reinterpret_cast<const real*>(a.Om) + nxt, LINES * NX * (unsigned)sizeof(real));
+        if (a.De) prefetch_l2_bulk(reinterpret_cast<const real*>(a.De) + nxt, LINES * NX * (unsigned)sizeof(real));
+      }
     }
-  } else {
+
+    if (MODE == MODE_PRO || MODE == MODE_FWD) {
 #pragma unroll
-    for (int g = 0; g < P::G; ++g)
+      for (int n = 0; n < 16; ++n) v[n] = St::ld(a.src, (rowbase + t + n * T) * 2 + c);
+      if (MODE == MODE_PRO && a.scale != nullptr) {
+        const double s = a.scale[c];
 #pragma unroll
-      for (int s = 0; s < P::RL; ++s)
-        v[g * P::RL + s] = St::ld(a.src, (rowbase + (t + g * T) + (NX / P::RL) * s) * 2 + c);
-    line_fft_inv<NX>(buf, a.tw, t, c, v);
+        for (int n = 0; n < 16; ++n) v[n] = mk(v[n].re * s, v[n].im * s);
+      }
+    } else {
+#pragma unroll
+      for (int g = 0; g < P::G; ++g)
+#pragma unroll
+        for (int s = 0; s < P::RL; ++s)
+          v[g * P::RL + s] = St::ld(a.src, (rowbase + (t + g * T) + (NX / P::RL) * s) * 2 + c);
+      line_fft_inv<NX>(buf, a.tw, t, c, v);
+    }
+
+    if (MODE != MODE_FWD) {
+      // the exchange buffer is idle during the real-space part: it holds the field rows meanwhile
+      __syncthreads();
+      stage_fields<DT, NX, LINES>(smem, a, first_point, tid);
+      cp_async_wait_all();
+      __syncthreads();
+      real_space<DT, NX, LINES, MODE>(v, a, smem, line, t, c, su, sd);
+      __syncthreads();
+    }
+
+    if (MODE == MODE_EPI) {
+#pragma unroll
+      for (int n = 0; n < 16; ++n) St::st(a.dst, (rowbase + t + n * T) * 2 + c, v[n]);
+    } else {
+      line_fft_fwd<NX>(buf, a.tw, t, c, v);
+#pragma unroll
+      for (int g = 0; g < P::G; ++g)
+#pragma unroll
+        for (int s = 0; s < P::RL; ++s) {
+          const int pos = (t + g * T) + (NX / P::RL) * s;
+          cplx o = v[g * P::RL + s];
+          if (MODE != MODE_FWD) {
+            double2 e = __ldg(a.exk + c * NX + pos + late_zero(o.re));
+            o = cmul(o, mk(e.x, e.y));
+          }
+          St::st(a.dst, (rowbase + pos) * 2 + c, o);
+        }
+      __syncthreads();  // the last exchange has been read by every warp before the next group writes
+    }
   }
 
-  double su = 0.0, sd = 0.0;
-  if (MODE != MODE_FWD) real_space<DT, NX, MODE>(v, a, rowbase, t, c, su, sd);
-
-  if (MODE == MODE_EPI) {
+  if (MODE == MODE_EPI && a.want_norm) {
+    // the c=0 thread of a pair summed points n<8, the c=1 thread n>=8: add over the whole CTA
+    __shared__ double red[2][32];
 #pragma unroll
-    for (int n = 0; n < 16; ++n) St::st(a.dst, (rowbase + t + n * T) * 2 + c, v[n]);
-    if (a.want_norm) {
-      // the c=0 thread of a pair summed points n<8, the c=1 thread n>=8: add over the whole CTA
-      __shared__ double red[2][32];
-#pragma unroll
-      for (int m = 16; m >= 1; m >>= 1) {
-        su += shfl_xor_d(su, m);
-        sd += shfl_xor_d(sd, m);
-      }
-      const int w = tid >> 5, nw = (blockDim.x + 31) >> 5;
-      if ((tid & 31) == 0) { red[0][w] = su; red[1][w] = sd; }
-      __syncthreads();
-      if (tid == 0) {
-        double s0 = 0.0, s1 = 0.0;
-        for (int i = 0; i < nw; ++i) { s0 += red[0][i]; s1 += red[1][i]; }
-        a.partial[2 * blockIdx.x] = s0;
-        a.partial[2 * blockIdx.x + 1] = s1;
-      }
+    for (int m = 16; m >= 1; m >>= 1) {
+      su += shfl_xor_d(su, m);
+      sd += shfl_xor_d(sd, m);
     }
-  } else {
-    line_fft_fwd<NX>(buf, a.tw, t, c, v);
-#pragma unroll
-    for (int g = 0; g < P::G; ++g)
-#pragma unroll
-      for (int s = 0; s < P::RL; ++s) {
-        const int pos = (t + g * T) + (NX / P::RL) * s;
-        cplx o = v[g * P::RL + s];
-        if (MODE != MODE_FWD) {
-          double2 e = __ldg(a.exk + c * NX + pos + late_zero(o.re));
-          o = cmul(o, mk(e.x, e.y));
-        }
-        St::st(a.dst, (rowbase + pos) * 2 + c, o);
-      }
+    const int w = tid >> 5, nw = (blockDim.x + 31) >> 5;
+    if ((tid & 31) == 0) { red[0][w] = su; red[1][w] = sd; }
+    __syncthreads();
+    if (tid == 0) {
+      double s0 = 0.0, s1 = 0.0;
+      for (int i = 0; i < nw; ++i) { s0 += red[0][i]; s1 += red[1][i]; }
+      a.partial[2 * blockIdx.x] = s0;
+      a.partial[2 * blockIdx.x + 1] = s1;
+    }
   }
 }
 

@@ -8,22 +8,22 @@
 namespace spgpe {
 
 namespace {
-struct PlanInfo { int ns, rl, lines; };
+struct PlanInfo { int ns, rl, lines_y; };
 PlanInfo plan_info(int n) {
   switch (n) {
-    case 64: return {Plan<64>::NS, Plan<64>::RL, Lines<64>::X};
-    case 128: return {Plan<128>::NS, Plan<128>::RL, Lines<128>::X};
-    case 256: return {Plan<256>::NS, Plan<256>::RL, Lines<256>::X};
-    case 512: return {Plan<512>::NS, Plan<512>::RL, Lines<512>::X};
-    case 1024: return {Plan<1024>::NS, Plan<1024>::RL, Lines<1024>::X};
-    case 2048: return {Plan<2048>::NS, Plan<2048>::RL, Lines<2048>::X};
-    case 4096: return {Plan<4096>::NS, Plan<4096>::RL, Lines<4096>::X};
+    case 64: return {Plan<64>::NS, Plan<64>::RL, Lines<64>::Y};
+    case 128: return {Plan<128>::NS, Plan<128>::RL, Lines<128>::Y};
+    case 256: return {Plan<256>::NS, Plan<256>::RL, Lines<256>::Y};
+    case 512: return {Plan<512>::NS, Plan<512>::RL, Lines<512>::Y};
+    case 1024: return {Plan<1024>::NS, Plan<1024>::RL, Lines<1024>::Y};
+    case 2048: return {Plan<2048>::NS, Plan<2048>::RL, Lines<2048>::Y};
+    case 4096: return {Plan<4096>::NS, Plan<4096>::RL, Lines<4096>::Y};
     default: return {0, 0, 0};
   }
 }
 }  // namespace
 
-int plan_lines(int n) { return plan_info(n).lines; }
+int plan_lines_y(int n) { return plan_info(n).lines_y; }
 
 int plan_tw_total(int n) {
   PlanInfo p = plan_info(n);
