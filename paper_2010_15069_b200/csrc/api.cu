@@ -2,6 +2,7 @@
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
+#include <stdlib.h>
 
 #include <new>
 #include <vector>
@@ -29,9 +30,11 @@ struct spgpe_ctx {
   int tab_imag;
   bool tab_valid;
   double *partial, *scale, *target, *dout;
+  double* fmax;  // [3] max |V|, |Omega|, |delta| (tier bounds of the row pass)
   int partial_cap;
   bool ready;
   long long launches;
+  int ygrid;  // CTAs of the last column-pass launch
   int xgrid;  // CTAs of the last row-pass launch (rows of `partial` it wrote)
   HalfCoef hc;
   // per-launch CUDA-event timing (spgpe_profile): pairs of events around every row/column pass launch
@@ -90,13 +93,13 @@ static cudaError_t dispatch_x_raw(spgpe_ctx* h, int mode, const PassXArgs& a) {
 }
 static cudaError_t dispatch_y_raw(spgpe_ctx* h, int ymode, const PassYArgs& a) {
   switch (h->ny) {
-    case 64: return launch_pass_y_64(h->dt, ymode, a, h->stream);
-    case 128: return launch_pass_y_128(h->dt, ymode, a, h->stream);
-    case 256: return launch_pass_y_256(h->dt, ymode, a, h->stream);
-    case 512: return launch_pass_y_512(h->dt, ymode, a, h->stream);
-    case 1024: return launch_pass_y_1024(h->dt, ymode, a, h->stream);
-    case 2048: return launch_pass_y_2048(h->dt, ymode, a, h->stream);
-    default: return launch_pass_y_4096(h->dt, ymode, a, h->stream);
+    case 64: return launch_pass_y_64(h->dt, ymode, a, h->stream, &h->ygrid);
+    case 128: return launch_pass_y_128(h->dt, ymode, a, h->stream, &h->ygrid);
+    case 256: return launch_pass_y_256(h->dt, ymode, a, h->stream, &h->ygrid);
+    case 512: return launch_pass_y_512(h->dt, ymode, a, h->stream, &h->ygrid);
+    case 1024: return launch_pass_y_1024(h->dt, ymode, a, h->stream, &h->ygrid);
+    case 2048: return launch_pass_y_2048(h->dt, ymode, a, h->stream, &h->ygrid);
+    default: return launch_pass_y_4096(h->dt, ymode, a, h->stream, &h->ygrid);
   }
 }
 
@@ -188,6 +191,8 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
   alloc((void**)&h->scale, sizeof(double) * 2);
   alloc((void**)&h->target, sizeof(double) * 2);
   alloc((void**)&h->dout, sizeof(double) * 8);
+  alloc((void**)&h->fmax, sizeof(double) * 3);
+  if (e == cudaSuccess) e = cudaMemset(h->fmax, 0, sizeof(double) * 3);
   if (e == cudaSuccess) {
     std::vector<double2> tw(twx > twy ? twx : twy);
     plan_fill_twiddles(nx, tw.data());
@@ -215,7 +220,7 @@ extern "C" int spgpe_destroy(spgpe_handle h) {
   if (!h) return SPGPE_ERR_INVALID_ARG;
   cudaStreamSynchronize(h->stream);
   void* ptrs[] = {h->psi, h->scratch, h->Vbuf, h->Ombuf, h->Debuf, h->tw_x, h->tw_y, h->Kx, h->Ky,
-                  h->exk, h->eyk, h->partial, h->scale, h->target, h->dout};
+                  h->exk, h->eyk, h->partial, h->scale, h->target, h->dout, h->fmax};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   if (h->prof_ev) {
@@ -229,13 +234,17 @@ extern "C" int spgpe_destroy(spgpe_handle h) {
 
 static int set_field(spgpe_handle h, const void* src, void* buf, const void** slot, cudaMemcpyKind kind) {
   if (!h) return SPGPE_ERR_INVALID_ARG;
+  const int which = (buf == h->Vbuf) ? 0 : (buf == h->Ombuf ? 1 : 2);
   if (!src) {
     *slot = nullptr;
+    CK(aux_absmax(h->dt, nullptr, 0, h->fmax + which, h->stream));
     return SPGPE_OK;
   }
   CK(cudaMemcpyAsync(buf, src, h->field_bytes, kind, h->stream));
   if (kind == cudaMemcpyHostToDevice) CK(cudaStreamSynchronize(h->stream));
   *slot = buf;
+  h->launches++;
+  CK(aux_absmax(h->dt, buf, h->points, h->fmax + which, h->stream));
   return SPGPE_OK;
 }
 extern "C" int spgpe_set_potential(spgpe_handle h, const void* d) {
@@ -314,7 +323,7 @@ extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
   memset(&xa, 0, sizeof(xa));
   xa.src = h->psi; xa.dst = h->psi; xa.V = h->V; xa.Om = h->Om; xa.De = h->De;
   xa.tw = h->tw_x; xa.exk = h->exk; xa.scale = nullptr; xa.partial = h->partial;
-  xa.tau = 0.5 * dt; xa.hc = h->hc; xa.imag = imag; xa.want_norm = imag; xa.ny = h->ny;
+  xa.tau = 0.5 * dt; xa.hc = h->hc; xa.imag = imag; xa.want_norm = imag; xa.ny = h->ny; xa.fmax = h->fmax;
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
   ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx;
@@ -368,7 +377,7 @@ extern "C" int spgpe_energy(spgpe_handle h, double out[5]) {
   memset(&ya, 0, sizeof(ya));
   ya.psi = h->scratch; ya.tw = h->tw_y; ya.Kx = h->Kx; ya.Ky = h->Ky; ya.partial = h->partial; ya.nx = h->nx;
   CK(dispatch_y(h, YMODE_ENERGY, ya));
-  CK(aux_sum_partials(h->partial, h->nx / plan_lines_y(h->ny), 1, w / ((double)h->nx * (double)h->ny), h->dout + 1,
+  CK(aux_sum_partials(h->partial, h->ygrid, 1, w / ((double)h->nx * (double)h->ny), h->dout + 1,
                       h->stream));
   double tmp[5];
   CK(cudaMemcpyAsync(tmp + 1, h->dout + 1, 4 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));

@@ -172,6 +172,26 @@ cudaError_t aux_set_targets(double* target, double n_up, double n_dn, cudaStream
   return cudaGetLastError();
 }
 
+// ---- max |f| of a field (bounds for the tier choice of the row pass) -------------------------------------------
+// non-negative doubles order like their bit patterns, so the grid-wide maximum is an atomicMax on the bits
+template <int DT>
+__global__ void absmax_kernel(const void* f, size_t n, unsigned long long* out) {
+  typedef Store<DT> St;
+  double m = 0.0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    m = fmax(m, fabs(St::ldr(f, i)));
+#pragma unroll
+  for (int k = 16; k >= 1; k >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, k));
+  if ((threadIdx.x & 31) == 0) atomicMax(out, (unsigned long long)__double_as_longlong(m));
+}
+cudaError_t aux_absmax(int dt, const void* field, size_t points, double* out, cudaStream_t s) {
+  cudaError_t e = cudaMemsetAsync(out, 0, sizeof(double), s);
+  if (e != cudaSuccess || field == nullptr) return e;
+  if (dt == 0) absmax_kernel<0><<<296, 256, 0, s>>>(field, points, reinterpret_cast<unsigned long long*>(out));
+  else absmax_kernel<1><<<296, 256, 0, s>>>(field, points, reinterpret_cast<unsigned long long*>(out));
+  return cudaGetLastError();
+}
+
 // ---- peak probes ---------------------------------------------------------------------------------------------
 __global__ void dfma_probe_kernel(double* out, int iters) {
   double a0 = threadIdx.x * 1e-9, a1 = a0 + 1.0, a2 = a0 + 2.0, a3 = a0 + 3.0;

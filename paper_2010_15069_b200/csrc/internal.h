@@ -10,7 +10,7 @@ namespace spgpe {
 // per-length launchers (inst_<N>.cu)
 #define SPGPE_DECL(N_)                                                                          \
   cudaError_t launch_pass_x_##N_(int dt, int mode, const PassXArgs& a, int ny, cudaStream_t s, int* grid); \
-  cudaError_t launch_pass_y_##N_(int dt, int ymode, const PassYArgs& a, cudaStream_t s);
+  cudaError_t launch_pass_y_##N_(int dt, int ymode, const PassYArgs& a, cudaStream_t s, int* grid);
 SPGPE_DECL(64)
 SPGPE_DECL(128)
 SPGPE_DECL(256)
@@ -24,7 +24,6 @@ SPGPE_DECL(4096)
 int plan_tw_total(int n);                       // number of twiddle entries of length n
 void plan_fill_twiddles(int n, double2* host);  // exp(-2 pi i k lo / (16 M_j)) blocks, see common.cuh
 int plan_freq_of_pos(int n, int pos);           // signed-less frequency index f in [0, n) stored at position pos
-int plan_lines_y(int n);                        // columns per CTA of the column pass of length n
 
 // small kernels (aux.cu); all enqueue on s and return cudaGetLastError()
 cudaError_t aux_phase_tables(const double* Kx, const double* Ky, int nx, int ny, double dt, int imag,
@@ -44,6 +43,8 @@ cudaError_t aux_energy_partials(int dt, const void* psi, const void* V, const vo
                                 size_t points, double g_uu, double g_dd, double g_ud, double* partial,
                                 int nblk, cudaStream_t s);
 cudaError_t aux_set_targets(double* target, double n_up, double n_dn, cudaStream_t s);
+// out[0] = max |field| (0 for a NULL field)
+cudaError_t aux_absmax(int dt, const void* field, size_t points, double* out, cudaStream_t s);
 // probes (bench roofline denominators)
 cudaError_t aux_probe_dfma(cudaStream_t s, double* tflops);
 cudaError_t aux_probe_copy(cudaStream_t s, long long bytes, double* gbs);

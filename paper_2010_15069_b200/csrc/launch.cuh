@@ -1,6 +1,7 @@
 // launch.cuh -- launch configuration per line length and the macro that instantiates the row/column
 // pass kernels of one length in its own translation unit (inst_<N>.cu), so that lengths compile in parallel.
 #pragma once
+#include <stdlib.h>
 #include "pass_x.cuh"
 #include "pass_y.cuh"
 
@@ -22,6 +23,7 @@ cudaError_t resident_ctas(K kernel, int threads, size_t smem, int* out) {
   if (e != cudaSuccess) return e;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem);
   if (e != cudaSuccess) return e;
+  if (const char* cap = getenv("SPGPE_DEBUG_CTAS_PER_SM")) { int c = atoi(cap); if (c > 0 && c < occ) occ = c; }
   *out = sms * (occ > 0 ? occ : 1);
   return cudaSuccess;
 }
@@ -31,7 +33,7 @@ template <int DT, int N, int MODE>
 cudaError_t launch_x(const PassXArgs& a, int ny, cudaStream_t s, int* grid_out) {
   constexpr int L = Lines<N>::X;
   auto k = pass_x_kernel<DT, N, L, MODE>;
-  constexpr size_t smem = (size_t)L * Plan<N>::PTS * 2 * sizeof(double2);
+  constexpr size_t smem = XSmem<N, L>::BYTES;
   static int resident = 0;
   if (resident == 0) {
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -47,17 +49,21 @@ cudaError_t launch_x(const PassXArgs& a, int ny, cudaStream_t s, int* grid_out) 
 }
 
 template <int DT, int N, int YMODE>
-cudaError_t launch_y(const PassYArgs& a, cudaStream_t s) {
+cudaError_t launch_y(const PassYArgs& a, cudaStream_t s, int* grid_out) {
   constexpr int L = Lines<N>::Y;
   auto k = pass_y_kernel<DT, N, L, YMODE>;
-  constexpr size_t smem = (size_t)L * YLayout<N, L>::LINE_PTS * 2 * sizeof(double2);
-  static bool attr_set = false;
-  if (!attr_set) {
+  constexpr size_t smem = YSmem<N, L>::BYTES;
+  static int resident = 0;
+  if (resident == 0) {
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    attr_set = true;
+    e = resident_ctas(k, L * (N / 8), smem, &resident);
+    if (e != cudaSuccess) return e;
   }
-  k<<<a.nx / L, L * (N / 8), smem, s>>>(a);
+  const int groups = a.nx / L;
+  const int grid = groups < resident ? groups : resident;
+  *grid_out = grid;
+  k<<<grid, L * (N / 8), smem, s>>>(a);
   return cudaGetLastError();
 }
 
@@ -78,12 +84,12 @@ cudaError_t launch_y(const PassYArgs& a, cudaStream_t s) {
       default: return launch_x<1, N_, MODE_FWD>(a, ny, s, g);                                       \
     }                                                                                            \
   }                                                                                              \
-  cudaError_t launch_pass_y_##N_(int dt, int ymode, const PassYArgs& a, cudaStream_t s) {        \
+  cudaError_t launch_pass_y_##N_(int dt, int ymode, const PassYArgs& a, cudaStream_t s, int* g) { \
     if (dt == 0)                                                                                 \
-      return ymode == YMODE_STEP ? launch_y<0, N_, YMODE_STEP>(a, s)                             \
-                                 : launch_y<0, N_, YMODE_ENERGY>(a, s);                          \
-    return ymode == YMODE_STEP ? launch_y<1, N_, YMODE_STEP>(a, s)                               \
-                               : launch_y<1, N_, YMODE_ENERGY>(a, s);                            \
+      return ymode == YMODE_STEP ? launch_y<0, N_, YMODE_STEP>(a, s, g)                             \
+                                 : launch_y<0, N_, YMODE_ENERGY>(a, s, g);                          \
+    return ymode == YMODE_STEP ? launch_y<1, N_, YMODE_STEP>(a, s, g)                               \
+                               : launch_y<1, N_, YMODE_ENERGY>(a, s, g);                            \
   }
 
 }  // namespace spgpe

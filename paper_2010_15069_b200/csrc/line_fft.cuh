@@ -6,6 +6,13 @@
 // (host-side table, see tables.cu).  Inverse is the exact mirror (unnormalised: inverse(forward(x)) = N x).
 // Between the two no reordering is needed, so pointwise k-space factors are applied on registers.
 //
+// Three-stage plans (N >= 512): after the first radix-16 stage the line splits into 16 independent blocks of
+// N/16 points, each owned by the RL threads t with the same t / RL (times two components): these threads sit in
+// ONE warp, so the exchange between the second stage and the last one needs only __syncwarp().  The last-stage
+// groups of thread t = (hi, lo) are q = hi*16 + lo + g*RL (inside its own block).
+//
+// Twiddles are read from a table in shared memory (copied there once per CTA by the pass kernels).
+//
 // Shared-memory line buffer: point p of component c lives at double2 index (p + (p >> PADSHIFT))*2 + c.
 #pragma once
 #include "radix.cuh"
@@ -29,91 +36,159 @@ struct StagePos {
   __device__ __forceinline__ int pos(int n) const { return base + n * M; }
 };
 
+// first last-stage group of thread t; its groups are group0 + g * GSTEP
+template <int N>
+__device__ __forceinline__ int last_group0(int t) {
+  typedef Plan<N> P;
+  if (P::NS == 3) return (t / P::RL) * 16 + (t % P::RL);
+  return t;
+}
+template <int N> struct LastStep { static constexpr int GSTEP = (Plan<N>::NS == 3) ? Plan<N>::RL : Plan<N>::T; };
+
+// double2 index of element (group q0 + g*GSTEP, s) of the last stage.  When RL == 2^PADSHIFT the padded index is
+// affine in (g, s): one base per thread plus compile-time offsets.
+template <int N>
+struct LastIdx {
+  typedef Plan<N> P;
+  static constexpr bool AFFINE = (P::RL == (1 << P::PADSHIFT));
+  int base;
+  __device__ __forceinline__ LastIdx(int t, int c) {
+    const int q0 = last_group0<N>(t);
+    base = AFFINE ? (q0 * (P::RL + 1) * 2 + c) : (q0 * P::RL * 2 + c);
+    q0_ = q0; c_ = c;
+  }
+  __device__ __forceinline__ int at(int g, int s) const {
+    if (AFFINE) return base + (g * LastStep<N>::GSTEP * (P::RL + 1) + s) * 2;
+    return smem_idx<N>((q0_ + g * LastStep<N>::GSTEP) * P::RL + s, c_);
+  }
+  int q0_, c_;
+};
+
 template <int N>
 __device__ __forceinline__ void sts_last(double2* buf, int t, int c, const cplx* v) {
   typedef Plan<N> P;
+  const LastIdx<N> ix(t, c);
 #pragma unroll
   for (int g = 0; g < P::G; ++g)
 #pragma unroll
     for (int s = 0; s < P::RL; ++s)
-      buf[smem_idx<N>((t + g * P::T) * P::RL + s, c)] = make_double2(v[g * P::RL + s].re, v[g * P::RL + s].im);
+      buf[ix.at(g, s)] = make_double2(v[g * P::RL + s].re, v[g * P::RL + s].im);
 }
 template <int N>
 __device__ __forceinline__ void lds_last(const double2* buf, int t, int c, cplx* v) {
   typedef Plan<N> P;
+  const LastIdx<N> ix(t, c);
 #pragma unroll
   for (int g = 0; g < P::G; ++g)
 #pragma unroll
     for (int s = 0; s < P::RL; ++s) {
-      double2 d = buf[smem_idx<N>((t + g * P::T) * P::RL + s, c)];
+      double2 d = buf[ix.at(g, s)];
       v[g * P::RL + s] = mk(d.x, d.y);
     }
 }
+// barrier of the exchange next to the last stage: warp-local for three-stage plans
+template <int N>
+__device__ __forceinline__ void sync_last() {
+  if (Plan<N>::NS == 3) __syncwarp();
+  else __syncthreads();
+}
+// double2 index of element n of radix-16 stage J: affine in n when the stride M is a multiple of the padding period
+template <int N, int J>
+struct StageIdx {
+  static constexpr int M = N >> (4 * J);
+  static constexpr int S = Plan<N>::PADSHIFT;
+  static constexpr bool AFFINE = (M % (1 << S)) == 0;
+  StagePos<N, J> sp;
+  int base, c_;
+  __device__ __forceinline__ StageIdx(int t, int c) : sp(t), c_(c) { base = smem_idx<N>(sp.base, c); }
+  __device__ __forceinline__ int at(int n) const {
+    if (AFFINE) return base + n * ((M + (M >> S)) * 2);
+    return smem_idx<N>(sp.pos(n), c_);
+  }
+};
 template <int N, int J>
 __device__ __forceinline__ void sts_stage(double2* buf, int t, int c, const cplx* v) {
-  StagePos<N, J> sp(t);
+  const StageIdx<N, J> ix(t, c);
 #pragma unroll
-  for (int n = 0; n < 16; ++n) buf[smem_idx<N>(sp.pos(n), c)] = make_double2(v[n].re, v[n].im);
+  for (int n = 0; n < 16; ++n) buf[ix.at(n)] = make_double2(v[n].re, v[n].im);
 }
 template <int N, int J>
 __device__ __forceinline__ void lds_stage(const double2* buf, int t, int c, cplx* v) {
-  StagePos<N, J> sp(t);
+  const StageIdx<N, J> ix(t, c);
 #pragma unroll
   for (int n = 0; n < 16; ++n) {
-    double2 d = buf[smem_idx<N>(sp.pos(n), c)];
+    double2 d = buf[ix.at(n)];
     v[n] = mk(d.x, d.y);
   }
 }
 
 // v[k] *= w_j[k][lo] (forward) or conj (inverse); w_j[k][lo] = exp(-2 pi i k lo / (16 M_j))
+//
+// flip (0 or 0x80000000, stage 1 only) negates the twiddles of odd k.  With it a thread may hold its 16 points
+// rotated by 8 (register n = point (n + 8) mod 16) on the natural-order side of the transform: rotating the
+// input of a 16-point DFT by 8 multiplies output k by (-1)^k, and multiplying input k by (-1)^k rotates the output.
+__device__ __forceinline__ double flip_sign(double x, int flip) {
+  return __hiloint2double(__double2hiint(x) ^ flip, __double2loint(x));
+}
 template <int N, int J, int D>
-__device__ __forceinline__ void twiddle(const double2* __restrict__ tw, int t, cplx* v) {
+__device__ __forceinline__ void twiddle(const double2* tw, int t, cplx* v, int flip) {
   constexpr int M = N >> (4 * J);
   const int lo = t & (M - 1);
   const double2* w = tw + tw_offset<N>(J) + lo;
 #pragma unroll
   for (int k = 1; k < 16; ++k) {
-    // the address depends on v[k] (late_zero), so that ptxas cannot hoist the table load far above its use
-    double2 d = __ldg(w + (k - 1) * M + late_zero(v[k].re));
+    double2 d = w[(k - 1) * M];
+    if (J == 1 && (k & 1)) {
+      d.x = flip_sign(d.x, flip);
+      d.y = flip_sign(d.y, flip);
+    }
     v[k] = (D < 0) ? cmul(v[k], mk(d.x, d.y)) : cmulc(v[k], mk(d.x, d.y));
   }
 }
 
 // one forward radix-16 stage J followed by the exchange into stage J+1's (or the last stage's) registers
 template <int N, int J>
-__device__ __forceinline__ void fwd_stages(double2* buf, const double2* __restrict__ tw, int t, int c, cplx* v) {
+__device__ __forceinline__ void fwd_stages(double2* buf, const double2* tw, int t, int c, cplx* v, int flip) {
   if constexpr (J < Plan<N>::NS) {
     dft16<-1>(v);
-    twiddle<N, J, -1>(tw, t, v);
+    twiddle<N, J, -1>(tw, t, v, flip);
     sts_stage<N, J>(buf, t, c, v);
-    __syncthreads();
-    if constexpr (J + 1 < Plan<N>::NS) lds_stage<N, J + 1>(buf, t, c, v);
-    else lds_last<N>(buf, t, c, v);
-    fwd_stages<N, J + 1>(buf, tw, t, c, v);
+    if constexpr (J + 1 < Plan<N>::NS) {
+      __syncthreads();
+      lds_stage<N, J + 1>(buf, t, c, v);
+    } else {
+      sync_last<N>();
+      lds_last<N>(buf, t, c, v);
+    }
+    fwd_stages<N, J + 1>(buf, tw, t, c, v, flip);
   }
 }
 template <int N>
-__device__ __forceinline__ void line_fft_fwd(double2* buf, const double2* __restrict__ tw, int t, int c, cplx* v) {
-  fwd_stages<N, 1>(buf, tw, t, c, v);
+__device__ __forceinline__ void line_fft_fwd(double2* buf, const double2* tw, int t, int c, cplx* v, int flip = 0) {
+  fwd_stages<N, 1>(buf, tw, t, c, v, flip);
   dft_last<-1, Plan<N>::RL>(v);
 }
 
 template <int N, int J>
-__device__ __forceinline__ void inv_stages(double2* buf, const double2* __restrict__ tw, int t, int c, cplx* v) {
+__device__ __forceinline__ void inv_stages(double2* buf, const double2* tw, int t, int c, cplx* v, int flip) {
   if constexpr (J >= 1) {
-    if constexpr (J + 1 < Plan<N>::NS) sts_stage<N, J + 1>(buf, t, c, v);
-    else sts_last<N>(buf, t, c, v);
-    __syncthreads();
+    if constexpr (J + 1 < Plan<N>::NS) {
+      sts_stage<N, J + 1>(buf, t, c, v);
+      __syncthreads();
+    } else {
+      sts_last<N>(buf, t, c, v);
+      sync_last<N>();
+    }
     lds_stage<N, J>(buf, t, c, v);
-    twiddle<N, J, +1>(tw, t, v);
+    twiddle<N, J, +1>(tw, t, v, flip);
     dft16<+1>(v);
-    inv_stages<N, J - 1>(buf, tw, t, c, v);
+    inv_stages<N, J - 1>(buf, tw, t, c, v, flip);
   }
 }
 template <int N>
-__device__ __forceinline__ void line_fft_inv(double2* buf, const double2* __restrict__ tw, int t, int c, cplx* v) {
+__device__ __forceinline__ void line_fft_inv(double2* buf, const double2* tw, int t, int c, cplx* v, int flip = 0) {
   dft_last<+1, Plan<N>::RL>(v);
-  inv_stages<N, Plan<N>::NS - 1>(buf, tw, t, c, v);
+  inv_stages<N, Plan<N>::NS - 1>(buf, tw, t, c, v, flip);
 }
 
 }  // namespace spgpe

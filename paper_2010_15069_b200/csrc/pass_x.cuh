@@ -33,6 +33,7 @@ struct PassXArgs {
   int imag;
   int want_norm;
   int ny;                // number of rows
+  const double* fmax;    // [3] device: max |V|, max |Omega|, max |delta| over the grid (tier bounds)
 };
 
 __device__ __forceinline__ double shfl_xor_d(double x, int m) { return __shfl_xor_sync(0xffffffffu, x, m); }
@@ -61,59 +62,91 @@ __device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, siz
   }
 }
 
-// Real-space part on the thread's registers v[n] = psi_c(x = t + n*T).  Pair exchange: the c=0 thread takes both
-// components of the points n = 0..7, the c=1 thread those of n = 8..15.  Fields come from shared memory
-// (stage_fields), index lx = line*NX + x.
-template <int DT, int NX, int LINES, int MODE>
-__device__ __forceinline__ void real_space(cplx* v, const PassXArgs& a, const void* fbuf, int line, int t, int c,
-                                           double& su, double& sd) {
+// Real-space part.  Register layout on the natural-order side (see twiddle(), flip): the lane of component c at
+// thread position t holds in v[i], i < 8, its component at "its" points x = t + (i + 8c) T and in v[8 + i] its
+// component at the partner lane's points.  For point i a lane receives the partner's v[8 + i] (the other
+// component at its own point), evaluates the half-step(s) in the (mine, other) basis (su2.cuh, LaneCoef) and
+// sends the other component back.  Fields come from shared memory (stage_fields), index lx = line*NX + x.
+// TIER: evaluation tier of su2.cuh, guaranteed by the caller for every point of the warp.
+template <int DT, int NX, int LINES, int MODE, int TIER>
+__device__ __forceinline__ void real_space_tier(cplx* v, const PassXArgs& a, const void* fbuf, int line, int t, int c,
+                                                const LaneCoef& lc, double& sm, double& so) {
   typedef Store<DT> St;
   typedef typename St::real real;
   constexpr int T = NX / 16;
-  const real* fV = reinterpret_cast<const real*>(fbuf);
+  const real* fV = reinterpret_cast<const real*>(fbuf) + line * NX + t + 8 * c * T;
   const real* fO = fV + LINES * NX;
   const real* fD = fO + LINES * NX;
   const double tau = a.tau, tau2 = a.tau * a.tau;
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
-    // send what the partner needs, receive the partner's component at my points
-    cplx mine = c ? v[8 + i] : v[i];
-    cplx send = c ? v[i] : v[8 + i];
-    cplx recv = shfl_xor_c(send, 1);
-    cplx up = c ? recv : mine;
-    cplx dn = c ? mine : recv;
-    const int lx = line * NX + t + (i + 8 * c) * T;
-    const double Vv = St::lds(fV, lx);
-    const double hO = 0.5 * St::lds(fO, lx);
-    const double hD = 0.5 * St::lds(fD, lx);
+    cplx m = v[i];
+    cplx o = shfl_xor_c(v[8 + i], 1);
+    const double Vv = St::lds(fV, i * T);
+    const double hO = 0.5 * St::lds(fO, i * T);
+    const double hD = lc.hs * St::lds(fD, i * T);
     if (MODE == MODE_MID) {
-      double a1 = su2_apply<false>(up, dn, Vv, hO, hD, tau, tau2, a.hc);
-      double a2 = su2_apply<false>(up, dn, Vv, hO, hD, tau, tau2, a.hc);
+      const double a1 = su2_apply<false, TIER>(m, o, Vv, hO, hD, tau, tau2, lc);
+      const double a2 = su2_apply<false, TIER>(m, o, Vv, hO, hD, tau, tau2, lc);
       double pr, pi;
-      phase_eval((a1 + a2) * tau, pr, pi);
-      apply_phase(up, dn, pr, pi);
+      phase_eval<TIER>((a1 + a2) * tau, pr, pi);
+      apply_phase(m, o, pr, pi);
     } else if (a.imag) {
-      double a1 = su2_apply<true>(up, dn, Vv, hO, hD, tau, tau2, a.hc);
-      double e = exp(-a1 * tau);
-      up = mk(up.re * e, up.im * e);
-      dn = mk(dn.re * e, dn.im * e);
+      const double a1 = su2_apply<true, TIER>(m, o, Vv, hO, hD, tau, tau2, lc);
+      const double e = exp(-a1 * tau);
+      m = mk(m.re * e, m.im * e);
+      o = mk(o.re * e, o.im * e);
     } else {
-      double a1 = su2_apply<false>(up, dn, Vv, hO, hD, tau, tau2, a.hc);
+      const double a1 = su2_apply<false, TIER>(m, o, Vv, hO, hD, tau, tau2, lc);
       double pr, pi;
-      phase_eval(a1 * tau, pr, pi);
-      apply_phase(up, dn, pr, pi);
+      phase_eval<TIER>(a1 * tau, pr, pi);
+      apply_phase(m, o, pr, pi);
     }
     if (MODE == MODE_EPI) {
-      su += fma(up.re, up.re, up.im * up.im);
-      sd += fma(dn.re, dn.re, dn.im * dn.im);
+      sm += fma(m.re, m.re, m.im * m.im);
+      so += fma(o.re, o.re, o.im * o.im);
     }
-    // give the partner its component back
-    cplx keep = c ? dn : up;
-    cplx back = shfl_xor_c(c ? up : dn, 1);
-    if (c) { v[8 + i] = keep; v[i] = back; }
-    else   { v[i] = keep; v[8 + i] = back; }
+    v[i] = m;
+    v[8 + i] = shfl_xor_c(o, 1);
   }
 }
+
+// Tier of the warp for this row, from bounds that hold for every point the warp touches:
+//   n_up + n_dn <= NT = max_n |own v[n]|^2 + the partner's maximum (conserved by the real-time half-step),
+//   |b_z| <= max|delta|/2 + max(|cbm|, |cbo|) NT,  |b_x| <= max|Omega|/2,  |a| <= max|V| + max(|cam|, |cao|) NT.
+template <int MODE>
+__device__ __forceinline__ int row_tier(const cplx* v, const PassXArgs& a, const LaneCoef& lc) {
+  double nmax = 0.0;
+#pragma unroll
+  for (int n = 0; n < 16; ++n) nmax = fmax(nmax, fma(v[n].re, v[n].re, v[n].im * v[n].im));
+  const double NT = nmax + shfl_xor_d(nmax, 1);
+  const double bz = fma(fmax(fabs(lc.cbm), fabs(lc.cbo)), NT, 0.5 * a.fmax[2]);
+  const double bx = 0.5 * a.fmax[1];
+  const double z = (a.tau * a.tau) * fma(bx, bx, bz * bz);
+  const double x = (MODE == MODE_MID ? 2.0 : 1.0) * a.tau * fma(fmax(fabs(lc.cam), fabs(lc.cao)), NT, a.fmax[0]);
+  const bool ph_ok = (x * x <= SPGPE_Z_FAST);
+  const bool t0 = ph_ok && (z <= SPGPE_Z_TINY);  // NaN fails every test and lands in the general tier
+  const bool t1 = ph_ok && (z <= SPGPE_Z_FAST);
+  if (__all_sync(0xffffffffu, t0)) return 0;
+  if (__all_sync(0xffffffffu, t1)) return 1;
+  return 2;
+}
+
+template <int DT, int NX, int LINES, int MODE>
+__device__ __forceinline__ void real_space(cplx* v, const PassXArgs& a, const void* fbuf, int line, int t, int c,
+                                           const LaneCoef& lc, double& sm, double& so) {
+  const int tier = row_tier<MODE>(v, a, lc);
+  if (tier == 0) real_space_tier<DT, NX, LINES, MODE, 0>(v, a, fbuf, line, t, c, lc, sm, so);
+  else if (tier == 1) real_space_tier<DT, NX, LINES, MODE, 1>(v, a, fbuf, line, t, c, lc, sm, so);
+  else real_space_tier<DT, NX, LINES, MODE, 2>(v, a, fbuf, line, t, c, lc, sm, so);
+}
+
+// dynamic shared memory of the row pass: LINES padded line buffers, then the twiddle table
+template <int NX, int LINES>
+struct XSmem {
+  static constexpr int EBUF = LINES * Plan<NX>::PTS * 2;                 // double2 elements
+  static constexpr size_t BYTES = (size_t)(EBUF + tw_total<NX>()) * 16;
+};
 
 // Persistent: CTA b handles the row groups b, b + gridDim.x, ...; while one group is being transformed the next
 // one (psi rows and field rows) is requested into L2, so that its loads find the data there.
@@ -131,8 +164,14 @@ pass_x_kernel(const PassXArgs a) {
   const int line = (tid >> 1) / T;
   double2* buf = smem + (size_t)line * (P::PTS * 2);
   const int ngroups = a.ny / LINES;
-  double su = 0.0, sd = 0.0;
+  double sm = 0.0, so = 0.0;  // sums of |own component|^2 and |other component|^2 over this lane's points
+  const LaneCoef lc = lane_coef(a.hc, c);
+  const int flip = c ? (int)0x80000000 : 0;  // the odd lane keeps its points rotated by 8 (twiddle())
   cplx v[16];
+  // twiddle table of NX behind the line buffers, copied once per (persistent) CTA
+  double2* twS = smem + XSmem<NX, LINES>::EBUF;
+  for (int i = tid; i < tw_total<NX>(); i += LINES * (NX / 8)) twS[i] = a.tw[i];
+  __syncthreads();
 
   for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
     const size_t first_point = (size_t)grp * LINES * NX;  // first point of the CTA's rows
@@ -150,7 +189,7 @@ pass_x_kernel(const PassXArgs a) {
 
     if (MODE == MODE_PRO || MODE == MODE_FWD) {
 #pragma unroll
-      for (int n = 0; n < 16; ++n) v[n] = St::ld(a.src, (rowbase + t + n * T) * 2 + c);
+      for (int n = 0; n < 16; ++n) v[n] = St::ld(a.src, (rowbase + t + ((n + 8 * c) & 15) * T) * 2 + c);
       if (MODE == MODE_PRO && a.scale != nullptr) {
         const double s = a.scale[c];
 #pragma unroll
@@ -162,7 +201,7 @@ pass_x_kernel(const PassXArgs a) {
 #pragma unroll
         for (int s = 0; s < P::RL; ++s)
           v[g * P::RL + s] = St::ld(a.src, (rowbase + (t + g * T) + (NX / P::RL) * s) * 2 + c);
-      line_fft_inv<NX>(buf, a.tw, t, c, v);
+      line_fft_inv<NX>(buf, twS, t, c, v, flip);
     }
 
     if (MODE != MODE_FWD) {
@@ -171,33 +210,36 @@ pass_x_kernel(const PassXArgs a) {
       stage_fields<DT, NX, LINES>(smem, a, first_point, tid);
       cp_async_wait_all();
       __syncthreads();
-      real_space<DT, NX, LINES, MODE>(v, a, smem, line, t, c, su, sd);
+      real_space<DT, NX, LINES, MODE>(v, a, smem, line, t, c, lc, sm, so);
       __syncthreads();
     }
 
     if (MODE == MODE_EPI) {
 #pragma unroll
-      for (int n = 0; n < 16; ++n) St::st(a.dst, (rowbase + t + n * T) * 2 + c, v[n]);
+      for (int n = 0; n < 16; ++n) St::st(a.dst, (rowbase + t + ((n + 8 * c) & 15) * T) * 2 + c, v[n]);
     } else {
-      line_fft_fwd<NX>(buf, a.tw, t, c, v);
+      line_fft_fwd<NX>(buf, twS, t, c, v, flip);
+      // k_x phase table: one base per thread, pinned behind the last butterfly (late_zero)
+      const double2* ex = a.exk + c * NX + t + late_zero(v[0].re);
 #pragma unroll
       for (int g = 0; g < P::G; ++g)
 #pragma unroll
         for (int s = 0; s < P::RL; ++s) {
-          const int pos = (t + g * T) + (NX / P::RL) * s;
+          const int off = g * T + (NX / P::RL) * s;
           cplx o = v[g * P::RL + s];
           if (MODE != MODE_FWD) {
-            double2 e = __ldg(a.exk + c * NX + pos + late_zero(o.re));
+            double2 e = __ldg(ex + off);
             o = cmul(o, mk(e.x, e.y));
           }
-          St::st(a.dst, (rowbase + pos) * 2 + c, o);
+          St::st(a.dst, (rowbase + t + off) * 2 + c, o);
         }
       __syncthreads();  // the last exchange has been read by every warp before the next group writes
     }
   }
 
   if (MODE == MODE_EPI && a.want_norm) {
-    // the c=0 thread of a pair summed points n<8, the c=1 thread n>=8: add over the whole CTA
+    // each lane summed its own and the other component over its 8 points of every row: sort into (up, down)
+    double su = c ? so : sm, sd = c ? sm : so;
     __shared__ double red[2][32];
 #pragma unroll
     for (int m = 16; m >= 1; m >>= 1) {

@@ -21,7 +21,7 @@ struct PassYArgs {
   const double2* eyk;   // [NY] k_y phase in stored order (YMODE_STEP)
   const double* Kx;     // [2][nx] (k_x +- k_L)^2/2 in the row pass's stored order (YMODE_ENERGY)
   const double* Ky;     // [NY] k_y^2/2 in stored order (YMODE_ENERGY)
-  double* partial;      // [gridDim.x] (YMODE_ENERGY)
+  double* partial;      // [gridDim.x] sum over this CTA's columns (YMODE_ENERGY)
   int nx;
 };
 
@@ -33,54 +33,82 @@ struct YLayout {
   static constexpr int LINE_PTS = BASE + ((WANT - (BASE & 3)) & 3);
 };
 
+// dynamic shared memory of the column pass: LINES padded line buffers, the twiddle table, and (YMODE_STEP, when
+// it fits in 227 KB) the k_y phase table
+template <int NY, int LINES>
+struct YSmem {
+  static constexpr int EBUF = LINES * YLayout<NY, LINES>::LINE_PTS * 2;  // double2 elements
+  static constexpr int TW = tw_total<NY>();
+  static constexpr bool EY_SMEM = (size_t)(EBUF + TW + NY) * 16 <= 227u * 1024u;
+  static constexpr size_t BYTES = (size_t)(EBUF + TW + (EY_SMEM ? NY : 0)) * 16;
+};
+
+// Persistent: CTA b handles the column groups b, b + gridDim.x, ...
 template <int DT, int NY, int LINES, int YMODE>
 __global__ void __launch_bounds__(LINES * (NY / 8), (LINES * (NY / 8) <= 256) ? 2 : 1)
 pass_y_kernel(const PassYArgs a) {
   typedef Plan<NY> P;
   typedef Store<DT> St;
+  typedef YSmem<NY, LINES> SM;
   extern __shared__ double2 smem[];
   constexpr int T = P::T;
+  constexpr int NTHR = LINES * (NY / 8);
   const int tid = threadIdx.x;
   const int c = tid & 1;
   const int line = (tid >> 1) % LINES;
   const int t = (tid >> 1) / LINES;
   double2* buf = smem + (size_t)line * (YLayout<NY, LINES>::LINE_PTS * 2);
-  const size_t col = (size_t)blockIdx.x * LINES + line;
+  double2* twS = smem + SM::EBUF;
+  const double2* ey = a.eyk;
+  for (int i = tid; i < SM::TW; i += NTHR) twS[i] = a.tw[i];
+  if (YMODE == YMODE_STEP && SM::EY_SMEM) {
+    double2* eyS = twS + SM::TW;
+    for (int i = tid; i < NY; i += NTHR) eyS[i] = a.eyk[i];
+    ey = eyS;
+  }
+  __syncthreads();
   const size_t nx = (size_t)a.nx;
+  const int ngroups = a.nx / LINES;
+  const size_t estride = (size_t)T * nx * 2;  // rows of one thread are T*nx points apart
+  double e = 0.0;
   cplx v[16];
 
-  // element (row t, column col, component c); rows of one thread are T*nx points apart
-  const size_t e0 = ((size_t)t * nx + col) * 2 + c;
-  const size_t estride = (size_t)T * nx * 2;
+  for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+    const size_t col = (size_t)grp * LINES + line;
+    // element (row t, column col, component c)
+    const size_t e0 = ((size_t)t * nx + col) * 2 + c;
 #pragma unroll
-  for (int n = 0; n < 16; ++n) v[n] = St::ld(a.psi, e0 + n * estride);
+    for (int n = 0; n < 16; ++n) v[n] = St::ld(a.psi, e0 + n * estride);
 
-  line_fft_fwd<NY>(buf, a.tw, t, c, v);
+    line_fft_fwd<NY>(buf, twS, t, c, v);
 
-  if (YMODE == YMODE_STEP) {
+    if (YMODE == YMODE_STEP) {
 #pragma unroll
-    for (int g = 0; g < P::G; ++g)
+      for (int g = 0; g < P::G; ++g)
 #pragma unroll
-      for (int s = 0; s < P::RL; ++s) {
-        double2 e = __ldg(a.eyk + (t + g * T) + (NY / P::RL) * s + late_zero(v[g * P::RL + s].re));
-        v[g * P::RL + s] = cmul(v[g * P::RL + s], mk(e.x, e.y));
-      }
-    line_fft_inv<NY>(buf, a.tw, t, c, v);
-    // recompute the addresses instead of keeping 16 of them alive across both transforms
-    size_t e1 = e0;
-    asm volatile("" : "+l"(e1));
+        for (int s = 0; s < P::RL; ++s) {
+          const int pos = (t + g * T) + (NY / P::RL) * s;
+          double2 f = SM::EY_SMEM ? ey[pos] : __ldg(ey + pos + late_zero(v[g * P::RL + s].re));
+          v[g * P::RL + s] = cmul(v[g * P::RL + s], mk(f.x, f.y));
+        }
+      line_fft_inv<NY>(buf, twS, t, c, v);
 #pragma unroll
-    for (int n = 0; n < 16; ++n) St::st(a.psi, e1 + n * estride, v[n]);
-  } else {
-    const double kx = a.Kx[(size_t)c * nx + col];
-    double e = 0.0;
+      for (int n = 0; n < 16; ++n) St::st(a.psi, e0 + n * estride, v[n]);
+      __syncthreads();  // the last exchange has been read by every warp before the next group writes
+    } else {
+      const double kx = a.Kx[(size_t)c * nx + col];
 #pragma unroll
-    for (int g = 0; g < P::G; ++g)
+      for (int g = 0; g < P::G; ++g)
 #pragma unroll
-      for (int s = 0; s < P::RL; ++s) {
-        const cplx z = v[g * P::RL + s];
-        e = fma(kx + a.Ky[(t + g * T) + (NY / P::RL) * s], fma(z.re, z.re, z.im * z.im), e);
-      }
+        for (int s = 0; s < P::RL; ++s) {
+          const cplx z = v[g * P::RL + s];
+          e = fma(kx + a.Ky[(t + g * T) + (NY / P::RL) * s], fma(z.re, z.re, z.im * z.im), e);
+        }
+      __syncthreads();
+    }
+  }
+
+  if (YMODE == YMODE_ENERGY) {
     __shared__ double red[32];
 #pragma unroll
     for (int m = 16; m >= 1; m >>= 1) e += __shfl_xor_sync(0xffffffffu, e, m);

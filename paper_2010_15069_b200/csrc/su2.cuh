@@ -7,10 +7,12 @@
 // and S(z) = sum z^k/(2k+1)! (sin theta/theta, sinh theta/theta).  Imaginary time: e^{-a tau}[C(z) 1 - tau S(z)(b.sigma)],
 // z = +theta^2.  Writing sin(theta)/|b| = tau S(z) needs no square root, no division and no |b| -> 0 special case.
 //
-// Evaluation tiers (the choice is warp-uniform, so there is no divergence):
+// Evaluation tiers:
 //   |z| <= 2^-13 : series to degree 3 (first dropped term z^4/8! < 6e-21)
 //   |z| <= 1/4   : series to degree 7 (first dropped term z^8/16! < 8e-19)
 //   otherwise    : libm sincos / cosh / sinh
+// The tier is chosen once per warp and row from rigorous bounds on |z| (pass_x.cuh), so the per-point code is
+// straight-line.
 #pragma once
 #include "common.cuh"
 
@@ -51,10 +53,11 @@ __device__ __forceinline__ void cs_series7(double z, double& C, double& S) {
   S = fma(s, z, 1.0);
 }
 
-// general argument: z = -theta^2 (real time, IMAG = false) or +theta^2 (imaginary time)
+// general argument: z = -theta^2 (real time, IMAG = false) or +theta^2 (imaginary time); returns (C, S)
 template <bool IMAG>
-__device__ __noinline__ void cs_general(double z, double& C, double& S) {
-  double th = sqrt(fabs(z));
+__device__ __noinline__ double2 cs_general(double z) {
+  double C, S;
+  const double th = sqrt(fabs(z));
   if (fabs(z) <= SPGPE_Z_FAST) {
     cs_series7(z, C, S);
   } else if (!IMAG) {
@@ -66,69 +69,86 @@ __device__ __noinline__ void cs_general(double z, double& C, double& S) {
     C = cosh(th);
     S = sinh(th) / th;
   }
+  return make_double2(C, S);
 }
 
-// tier of a warp: 0 tiny, 1 fast, 2 general (the largest |z| among the lanes decides)
-__device__ __forceinline__ int cs_tier(double absz) {
-  if (!__any_sync(0xffffffffu, absz > SPGPE_Z_TINY)) return 0;
-  if (!__any_sync(0xffffffffu, absz > SPGPE_Z_FAST)) return 1;
-  return 2;
-}
-
-template <bool IMAG>
+// TIER 0: |z| <= SPGPE_Z_TINY guaranteed by the caller; 1: |z| <= SPGPE_Z_FAST guaranteed; 2: anything
+template <bool IMAG, int TIER>
 __device__ __forceinline__ void cs_eval(double z, double& C, double& S) {
-  const int tier = cs_tier(fabs(z));
-  if (tier == 0) cs_series3(z, C, S);
-  else if (tier == 1) cs_series7(z, C, S);
-  else cs_general<IMAG>(z, C, S);
+  if (TIER == 0) {
+    cs_series3(z, C, S);
+  } else if (TIER == 1) {
+    cs_series7(z, C, S);
+  } else {
+    const double2 r = cs_general<IMAG>(z);
+    C = r.x;
+    S = r.y;
+  }
 }
 
-// e^{-i x}: (cos x, -sin x)
-static __device__ __noinline__ void phase_general(double x, double& pr, double& pi) {
+// e^{-i x} = (cos x, -sin x); TIER 0/1: x^2 <= SPGPE_Z_FAST guaranteed by the caller (series to degree 7)
+static __device__ __noinline__ double2 phase_general(double x) {
   double sn, cn;
   sincos(x, &sn, &cn);
-  pr = cn;
-  pi = -sn;
+  return make_double2(cn, -sn);
 }
+template <int TIER>
 __device__ __forceinline__ void phase_eval(double x, double& pr, double& pi) {
-  const double z = -(x * x);
-  const int tier = cs_tier(-z);
-  if (tier == 2) {
-    phase_general(x, pr, pi);
+  if (TIER == 2) {
+    const double2 r = phase_general(x);
+    pr = r.x;
+    pi = r.y;
   } else {
     double C, S;
-    if (tier == 0) cs_series3(z, C, S);
-    else cs_series7(z, C, S);
+    cs_series7(-(x * x), C, S);
     pr = C;
     pi = -(x * S);
   }
 }
 
-// Apply the traceless part M = C 1 - (i) tau S (b.sigma) to (up, dn) with the densities of (up, dn);
-// returns a (the scalar part of H_loc) so that the caller applies e^{-i a tau} / e^{-a tau}.
-// hOm = Omega/2 and hDe = delta/2 are passed halved.
-template <bool IMAG>
-__device__ __forceinline__ double su2_apply(cplx& up, cplx& dn, double V, double hOm, double hDe, double tau,
-                                            double tau2, const HalfCoef& hc) {
-  const double nu = fma(up.re, up.re, up.im * up.im);
-  const double nd = fma(dn.re, dn.re, dn.im * dn.im);
-  const double a = fma(hc.ca_u, nu, fma(hc.ca_d, nd, V));
-  const double bz = fma(hc.cb_u, nu, fma(hc.cb_d, nd, hDe));
-  const double bx = hOm;
-  const double th2 = tau2 * fma(bx, bx, bz * bz);
+// Per-lane form of the local Hamiltonian.  A lane holds "its" component m (up for the even lane of a pair, down
+// for the odd one) and receives the other component o.  In the basis (m, o) the matrix keeps its form with
+//   a  = V + cam |m|^2 + cao |o|^2,   b_z = hDs + cbm |m|^2 + cbo |o|^2,   b_x = hO,
+// (even lane: cam = ca_u, cao = ca_d, cbm = cb_u, cbo = cb_d, hDs = +delta/2; odd lane: cam = ca_d, cao = ca_u,
+// cbm = -cb_d, cbo = -cb_u, hDs = -delta/2, because sigma_z changes sign when the basis order is swapped), so
+// no lane ever has to sort (m, o) into (up, down).
+struct LaneCoef {
+  double cam, cao, cbm, cbo;
+  double hs;  // +0.5 or -0.5: factor that turns delta into hDs
+};
+__device__ __forceinline__ LaneCoef lane_coef(const HalfCoef& hc, int c) {
+  LaneCoef l;
+  l.cam = c ? hc.ca_d : hc.ca_u;
+  l.cao = c ? hc.ca_u : hc.ca_d;
+  l.cbm = c ? -hc.cb_d : hc.cb_u;
+  l.cbo = c ? -hc.cb_u : hc.cb_d;
+  l.hs = c ? -0.5 : 0.5;
+  return l;
+}
+
+// Apply the traceless part M = C 1 - (i) tau S (b.sigma) to (m, o) with the densities of (m, o); returns a (the
+// scalar part of H_loc) so that the caller applies e^{-i a tau} / e^{-a tau}.
+template <bool IMAG, int TIER>
+__device__ __forceinline__ double su2_apply(cplx& m, cplx& o, double V, double hO, double hDs, double tau,
+                                            double tau2, const LaneCoef& lc) {
+  const double nm = fma(m.re, m.re, m.im * m.im);
+  const double no = fma(o.re, o.re, o.im * o.im);
+  const double a = fma(lc.cam, nm, fma(lc.cao, no, V));
+  const double bz = fma(lc.cbm, nm, fma(lc.cbo, no, hDs));
+  const double th2 = tau2 * fma(hO, hO, bz * bz);
   double C, S;
-  cs_eval<IMAG>(IMAG ? th2 : -th2, C, S);
+  cs_eval<IMAG, TIER>(IMAG ? th2 : -th2, C, S);
   const double ts = tau * S;
-  const double sx = ts * bx, sz = ts * bz;
-  // w_up = sz up + sx dn,  w_dn = sx up - sz dn
-  const cplx wu = mk(fma(sz, up.re, sx * dn.re), fma(sz, up.im, sx * dn.im));
-  const cplx wd = mk(fma(sx, up.re, -(sz * dn.re)), fma(sx, up.im, -(sz * dn.im)));
+  const double sx = ts * hO, sz = ts * bz;
+  // w_m = sz m + sx o,  w_o = sx m - sz o
+  const cplx wm = mk(fma(sz, m.re, sx * o.re), fma(sz, m.im, sx * o.im));
+  const cplx wo = mk(fma(sx, m.re, -(sz * o.re)), fma(sx, m.im, -(sz * o.im)));
   if (IMAG) {
-    up = mk(fma(C, up.re, -wu.re), fma(C, up.im, -wu.im));
-    dn = mk(fma(C, dn.re, -wd.re), fma(C, dn.im, -wd.im));
+    m = mk(fma(C, m.re, -wm.re), fma(C, m.im, -wm.im));
+    o = mk(fma(C, o.re, -wo.re), fma(C, o.im, -wo.im));
   } else {  // -i w = (w.im, -w.re)
-    up = mk(fma(C, up.re, wu.im), fma(C, up.im, -wu.re));
-    dn = mk(fma(C, dn.re, wd.im), fma(C, dn.im, -wd.re));
+    m = mk(fma(C, m.re, wm.im), fma(C, m.im, -wm.re));
+    o = mk(fma(C, o.re, wo.im), fma(C, o.im, -wo.re));
   }
   return a;
 }

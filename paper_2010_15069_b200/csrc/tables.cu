@@ -23,7 +23,6 @@ PlanInfo plan_info(int n) {
 }
 }  // namespace
 
-int plan_lines_y(int n) { return plan_info(n).lines_y; }
 
 int plan_tw_total(int n) {
   PlanInfo p = plan_info(n);
@@ -49,20 +48,21 @@ void plan_fill_twiddles(int n, double2* host) {
   }
 }
 
-// Stored position pos = q + (n/RL) * k_last, q = sum_{j<NS} k_j * (n / (16^j RL));  f = sum_j k_j 16^(j-1).
+// Frequency index held at stored position pos = (t + g*T) + (n/RL) * s (T = n/16 threads per component, thread t,
+// last-stage group g, output s of the last butterfly).  Decimation in frequency: the first stage's output index is
+// the least significant digit.  Two-stage plans: the group q = t + g*T is the first stage's output k1, f = k1 + 16 s.
+// Three-stage plans (line_fft.cuh): thread t = (hi, lo), hi = t / RL = k1, its groups hold k2 = lo + g*RL,
+// f = k1 + 16 k2 + 256 s.
 int plan_freq_of_pos(int n, int pos) {
   PlanInfo p = plan_info(n);
   const int groups = n / p.rl;
-  const int klast = pos / groups;
+  const int s = pos / groups;
   const int q = pos % groups;
-  int f = 0, w = 1;
-  for (int j = 1; j < p.ns; ++j) {
-    const int weight = (n >> (4 * j)) / p.rl;
-    const int kj = (q / weight) % 16;
-    f += kj * w;
-    w *= 16;
-  }
-  return f + klast * w;
+  if (p.ns == 2) return q + 16 * s;
+  const int T = n / 16;
+  const int t = q % T, g = q / T;
+  const int hi = t / p.rl, lo = t % p.rl;
+  return hi + 16 * (lo + g * p.rl) + 256 * s;
 }
 
 }  // namespace spgpe
