@@ -30,6 +30,7 @@ struct spgpe_ctx {
   int tab_imag;
   bool tab_valid;
   double *partial, *scale, *target, *dout;
+  int* sched;    // [4] work counters of the persistent kernels: row pass [0..1], column pass [2..3]
   double* fmax;  // [3] max |V|, |Omega|, |delta| (tier bounds of the row pass)
   int partial_cap;
   bool ready;
@@ -191,6 +192,8 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
   alloc((void**)&h->scale, sizeof(double) * 2);
   alloc((void**)&h->target, sizeof(double) * 2);
   alloc((void**)&h->dout, sizeof(double) * 8);
+  alloc((void**)&h->sched, sizeof(int) * 4);
+  if (e == cudaSuccess) e = cudaMemset(h->sched, 0, sizeof(int) * 4);
   alloc((void**)&h->fmax, sizeof(double) * 3);
   if (e == cudaSuccess) e = cudaMemset(h->fmax, 0, sizeof(double) * 3);
   if (e == cudaSuccess) {
@@ -220,7 +223,7 @@ extern "C" int spgpe_destroy(spgpe_handle h) {
   if (!h) return SPGPE_ERR_INVALID_ARG;
   cudaStreamSynchronize(h->stream);
   void* ptrs[] = {h->psi, h->scratch, h->Vbuf, h->Ombuf, h->Debuf, h->tw_x, h->tw_y, h->Kx, h->Ky,
-                  h->exk, h->eyk, h->partial, h->scale, h->target, h->dout, h->fmax};
+                  h->exk, h->eyk, h->partial, h->scale, h->target, h->dout, h->fmax, h->sched};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   if (h->prof_ev) {
@@ -323,10 +326,10 @@ extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
   memset(&xa, 0, sizeof(xa));
   xa.src = h->psi; xa.dst = h->psi; xa.V = h->V; xa.Om = h->Om; xa.De = h->De;
   xa.tw = h->tw_x; xa.exk = h->exk; xa.scale = nullptr; xa.partial = h->partial;
-  xa.tau = 0.5 * dt; xa.hc = h->hc; xa.imag = imag; xa.want_norm = imag; xa.ny = h->ny; xa.fmax = h->fmax;
+  xa.tau = 0.5 * dt; xa.hc = h->hc; xa.imag = imag; xa.want_norm = imag; xa.ny = h->ny; xa.fmax = h->fmax; xa.sched = h->sched;
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
-  ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx;
+  ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx; ya.sched = h->sched + 2;
   const double w = (h->Lx / h->nx) * (h->Ly / h->ny);
   if (!imag) {
     CK(dispatch_x(h, MODE_PRO, xa));
@@ -371,11 +374,11 @@ extern "C" int spgpe_energy(spgpe_handle h, double out[5]) {
   CK(aux_sum_partials(h->partial, nblk, 3, w, h->dout + 2, h->stream));
   PassXArgs xa;
   memset(&xa, 0, sizeof(xa));
-  xa.src = h->psi; xa.dst = h->scratch; xa.tw = h->tw_x; xa.ny = h->ny;
+  xa.src = h->psi; xa.dst = h->scratch; xa.tw = h->tw_x; xa.ny = h->ny; xa.sched = h->sched; xa.fmax = h->fmax;
   CK(dispatch_x(h, MODE_FWD, xa));
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
-  ya.psi = h->scratch; ya.tw = h->tw_y; ya.Kx = h->Kx; ya.Ky = h->Ky; ya.partial = h->partial; ya.nx = h->nx;
+  ya.psi = h->scratch; ya.tw = h->tw_y; ya.Kx = h->Kx; ya.Ky = h->Ky; ya.partial = h->partial; ya.nx = h->nx; ya.sched = h->sched + 2;
   CK(dispatch_y(h, YMODE_ENERGY, ya));
   CK(aux_sum_partials(h->partial, h->ygrid, 1, w / ((double)h->nx * (double)h->ny), h->dout + 1,
                       h->stream));

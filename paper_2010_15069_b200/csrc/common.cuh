@@ -64,6 +64,7 @@ template <> struct Store<0> {
   static __device__ __forceinline__ double lds(const void* base, int idx) {
     return reinterpret_cast<const double*>(base)[idx];
   }
+  static __device__ __forceinline__ cplx cv(double2 e) { return mk(e.x, e.y); }
 };
 template <> struct Store<1> {
   typedef float real;
@@ -81,6 +82,7 @@ template <> struct Store<1> {
   static __device__ __forceinline__ double lds(const void* base, int idx) {
     return (double)reinterpret_cast<const float*>(base)[idx];
   }
+  static __device__ __forceinline__ cplx cv(float2 e) { return mk((double)e.x, (double)e.y); }
 };
 
 // ---- asynchronous copies ------------------------------------------------------------------------------------
@@ -89,10 +91,31 @@ __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
   const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
 }
+// 8-byte variant (complex64 elements)
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_elem(double2* smem_dst, const double2* gsrc) { cp_async16(smem_dst, gsrc); }
+__device__ __forceinline__ void cp_async_elem(float2* smem_dst, const float2* gsrc) { cp_async8(smem_dst, gsrc); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 // ask L2 to fetch `bytes` (multiple of 16) starting at the 16-byte aligned address p; no registers, no scoreboard
 __device__ __forceinline__ void prefetch_l2_bulk(const void* p, unsigned bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
+// ---- dynamic work distribution of the persistent pass kernels -------------------------------------------------
+// sched[0] = number of groups handed out beyond the first gridDim.x, sched[1] = CTAs that have finished.  CTA b
+// starts with group b and then takes gridDim.x + atomicAdd(sched[0], 1), so that fast SMs take more groups than
+// slow ones.  The last CTA to finish resets both words for the next launch (launches on one stream are serial).
+__device__ __forceinline__ int sched_next(int* sched) { return (int)gridDim.x + atomicAdd(&sched[0], 1); }
+__device__ __forceinline__ void sched_finish(int* sched) {
+  __threadfence();
+  if (atomicAdd(&sched[1], 1) == (int)gridDim.x - 1) {
+    sched[0] = 0;
+    sched[1] = 0;
+    __threadfence();
+  }
 }
 
 // ---- transform plan: N = 16 * 16 * ... * R_LAST, every thread holds 16 points of one component ----

@@ -169,8 +169,14 @@ __device__ __forceinline__ void line_fft_fwd(double2* buf, const double2* tw, in
   dft_last<-1, Plan<N>::RL>(v);
 }
 
-template <int N, int J>
-__device__ __forceinline__ void inv_stages(double2* buf, const double2* tw, int t, int c, cplx* v, int flip) {
+struct NoHook {
+  __device__ __forceinline__ void operator()() const {}
+};
+// hook() runs right after the last read of the line buffer (the loads of stage 1): from there on the buffer is
+// free as soon as every warp has passed that point
+template <int N, int J, typename Hook>
+__device__ __forceinline__ void inv_stages(double2* buf, const double2* tw, int t, int c, cplx* v, int flip,
+                                           const Hook& hook) {
   if constexpr (J >= 1) {
     if constexpr (J + 1 < Plan<N>::NS) {
       sts_stage<N, J + 1>(buf, t, c, v);
@@ -180,15 +186,17 @@ __device__ __forceinline__ void inv_stages(double2* buf, const double2* tw, int 
       sync_last<N>();
     }
     lds_stage<N, J>(buf, t, c, v);
+    if constexpr (J == 1) hook();
     twiddle<N, J, +1>(tw, t, v, flip);
     dft16<+1>(v);
-    inv_stages<N, J - 1>(buf, tw, t, c, v, flip);
+    inv_stages<N, J - 1>(buf, tw, t, c, v, flip, hook);
   }
 }
-template <int N>
-__device__ __forceinline__ void line_fft_inv(double2* buf, const double2* tw, int t, int c, cplx* v, int flip = 0) {
+template <int N, typename Hook = NoHook>
+__device__ __forceinline__ void line_fft_inv(double2* buf, const double2* tw, int t, int c, cplx* v, int flip = 0,
+                                             const Hook& hook = Hook()) {
   dft_last<+1, Plan<N>::RL>(v);
-  inv_stages<N, Plan<N>::NS - 1>(buf, tw, t, c, v, flip);
+  inv_stages<N, Plan<N>::NS - 1>(buf, tw, t, c, v, flip, hook);
 }
 
 }  // namespace spgpe

@@ -33,6 +33,7 @@ struct PassXArgs {
   int imag;
   int want_norm;
   int ny;                // number of rows
+  int* sched;            // [2] device: work counter (common.cuh, sched_next)
   const double* fmax;    // [3] device: max |V|, max |Omega|, max |delta| over the grid (tier bounds)
 };
 
@@ -156,7 +157,9 @@ pass_x_kernel(const PassXArgs a) {
   typedef Plan<NX> P;
   typedef Store<DT> St;
   typedef typename St::real real;
+  typedef typename St::elem elem;
   extern __shared__ double2 smem[];
+  constexpr int NTHR = LINES * (NX / 8);
   constexpr int T = P::T;
   const int tid = threadIdx.x;
   const int c = tid & 1;
@@ -173,36 +176,45 @@ pass_x_kernel(const PassXArgs a) {
   for (int i = tid; i < tw_total<NX>(); i += LINES * (NX / 8)) twS[i] = a.tw[i];
   __syncthreads();
 
-  for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
-    const size_t first_point = (size_t)grp * LINES * NX;  // first point of the CTA's rows
-    const size_t rowbase = first_point + (size_t)line * NX;
-    if (tid == 0 && grp + (int)gridDim.x < ngroups) {
-      const size_t nxt = (size_t)(grp + gridDim.x) * LINES * NX;
-      prefetch_l2_bulk(reinterpret_cast<const typename St::elem*>(a.src) + nxt * 2,
-                       LINES * NX * 2 * (unsigned)sizeof(typename St::elem));
-      if (MODE != MODE_FWD) {
-        if (a.V) prefetch_l2_bulk(reinterpret_cast<const real*>(a.V) + nxt, LINES * NX * (unsigned)sizeof(real));
-        if (a.Om) prefetch_l2_bulk(reinterpret_cast<const real*>(a.Om) + nxt, LINES * NX * (unsigned)sizeof(real));
-        if (a.De) prefetch_l2_bulk(reinterpret_cast<const real*>(a.De) + nxt, LINES * NX * (unsigned)sizeof(real));
-      }
-    }
-
+  // The psi rows of a group travel global -> shared memory asynchronously (cp.async into the line buffers, which
+  // are idle at that time: slot (n, tid) holds register n of thread tid), issued one group ahead so that the
+  // transfer runs under the tail of the previous group instead of stalling the CTA at the head of this one.
+  elem* stg = reinterpret_cast<elem*>(smem);
+  auto issue_loads = [&](int grp) {
+    const size_t rb = ((size_t)grp * LINES + line) * NX;
+    const elem* src = reinterpret_cast<const elem*>(a.src);
     if (MODE == MODE_PRO || MODE == MODE_FWD) {
 #pragma unroll
-      for (int n = 0; n < 16; ++n) v[n] = St::ld(a.src, (rowbase + t + ((n + 8 * c) & 15) * T) * 2 + c);
-      if (MODE == MODE_PRO && a.scale != nullptr) {
-        const double s = a.scale[c];
-#pragma unroll
-        for (int n = 0; n < 16; ++n) v[n] = mk(v[n].re * s, v[n].im * s);
-      }
+      for (int n = 0; n < 16; ++n)
+        cp_async_elem(stg + n * NTHR + tid, src + (rb + t + ((n + 8 * c) & 15) * T) * 2 + c);
     } else {
 #pragma unroll
       for (int g = 0; g < P::G; ++g)
 #pragma unroll
         for (int s = 0; s < P::RL; ++s)
-          v[g * P::RL + s] = St::ld(a.src, (rowbase + (t + g * T) + (NX / P::RL) * s) * 2 + c);
-      line_fft_inv<NX>(buf, twS, t, c, v, flip);
+          cp_async_elem(stg + (g * P::RL + s) * NTHR + tid, src + (rb + (t + g * T) + (NX / P::RL) * s) * 2 + c);
     }
+  };
+  if ((int)blockIdx.x < ngroups) issue_loads(blockIdx.x);
+
+  __shared__ int next_s[2];  // group this CTA takes next (written by thread 0, double-buffered over iterations)
+  int it = 0;
+  for (int grp = blockIdx.x; grp < ngroups; ++it) {
+    const size_t first_point = (size_t)grp * LINES * NX;  // first point of the CTA's rows
+    const size_t rowbase = first_point + (size_t)line * NX;
+    // the next group is requested now and published before the last barrier of this iteration (latency hidden)
+    int nxt_req = 0;
+    if (tid == 0) nxt_req = sched_next(a.sched);
+    cp_async_wait_all();
+#pragma unroll
+    for (int n = 0; n < 16; ++n) v[n] = St::cv(stg[n * NTHR + tid]);
+    if (MODE == MODE_PRO && a.scale != nullptr) {
+      const double s = a.scale[c];
+#pragma unroll
+      for (int n = 0; n < 16; ++n) v[n] = mk(v[n].re * s, v[n].im * s);
+    }
+    __syncthreads();  // every thread has taken its staged values: the buffers may be overwritten
+    if (MODE == MODE_MID || MODE == MODE_EPI) line_fft_inv<NX>(buf, twS, t, c, v, flip);
 
     if (MODE != MODE_FWD) {
       // the exchange buffer is idle during the real-space part: it holds the field rows meanwhile
@@ -211,14 +223,23 @@ pass_x_kernel(const PassXArgs a) {
       cp_async_wait_all();
       __syncthreads();
       real_space<DT, NX, LINES, MODE>(v, a, smem, line, t, c, lc, sm, so);
+      if (MODE == MODE_EPI && tid == 0) next_s[it & 1] = nxt_req;
       __syncthreads();
     }
 
+    int nxt_grp;
     if (MODE == MODE_EPI) {
+      nxt_grp = next_s[it & 1];
+      if (nxt_grp < ngroups) issue_loads(nxt_grp);  // the line buffers are free after the real-space part
 #pragma unroll
       for (int n = 0; n < 16; ++n) St::st(a.dst, (rowbase + t + ((n + 8 * c) & 15) * T) * 2 + c, v[n]);
     } else {
-      line_fft_fwd<NX>(buf, twS, t, c, v, flip);
+      fwd_stages<NX, 1>(buf, twS, t, c, v, flip);
+      if (tid == 0) next_s[it & 1] = nxt_req;
+      __syncthreads();  // the last exchange has been read by every warp: the line buffers are free
+      nxt_grp = next_s[it & 1];
+      if (nxt_grp < ngroups) issue_loads(nxt_grp);
+      dft_last<-1, P::RL>(v);
       // k_x phase table: one base per thread, pinned behind the last butterfly (late_zero)
       const double2* ex = a.exk + c * NX + t + late_zero(v[0].re);
 #pragma unroll
@@ -233,9 +254,16 @@ pass_x_kernel(const PassXArgs a) {
           }
           St::st(a.dst, (rowbase + t + off) * 2 + c, o);
         }
-      __syncthreads();  // the last exchange has been read by every warp before the next group writes
     }
+    if (MODE != MODE_FWD && tid == 0 && nxt_grp < ngroups) {  // field rows of the next group: into L2
+      const size_t nxt = (size_t)nxt_grp * LINES * NX;
+      if (a.V) prefetch_l2_bulk(reinterpret_cast<const real*>(a.V) + nxt, LINES * NX * (unsigned)sizeof(real));
+      if (a.Om) prefetch_l2_bulk(reinterpret_cast<const real*>(a.Om) + nxt, LINES * NX * (unsigned)sizeof(real));
+      if (a.De) prefetch_l2_bulk(reinterpret_cast<const real*>(a.De) + nxt, LINES * NX * (unsigned)sizeof(real));
+    }
+    grp = nxt_grp;
   }
+  if (tid == 0) sched_finish(a.sched);
 
   if (MODE == MODE_EPI && a.want_norm) {
     // each lane summed its own and the other component over its 8 points of every row: sort into (up, down)

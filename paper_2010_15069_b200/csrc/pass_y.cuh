@@ -23,6 +23,7 @@ struct PassYArgs {
   const double* Ky;     // [NY] k_y^2/2 in stored order (YMODE_ENERGY)
   double* partial;      // [gridDim.x] sum over this CTA's columns (YMODE_ENERGY)
   int nx;
+  int* sched;           // [2] device: work counter (common.cuh, sched_next)
 };
 
 template <int NY, int LINES>
@@ -73,12 +74,31 @@ pass_y_kernel(const PassYArgs a) {
   double e = 0.0;
   cplx v[16];
 
-  for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+  // The columns of a group travel global -> shared memory asynchronously (cp.async into the line buffers while
+  // they are idle: slot (n, tid) holds register n of thread tid), issued one group ahead.
+  typedef typename St::elem elem;
+  elem* stg = reinterpret_cast<elem*>(smem);
+  auto issue_loads = [&](int grp) {
     const size_t col = (size_t)grp * LINES + line;
-    // element (row t, column col, component c)
-    const size_t e0 = ((size_t)t * nx + col) * 2 + c;
+    const elem* src = reinterpret_cast<const elem*>(a.psi) + ((size_t)t * nx + col) * 2 + c;
 #pragma unroll
-    for (int n = 0; n < 16; ++n) v[n] = St::ld(a.psi, e0 + n * estride);
+    for (int n = 0; n < 16; ++n) cp_async_elem(stg + n * NTHR + tid, src + n * estride);
+  };
+  if ((int)blockIdx.x < ngroups) issue_loads(blockIdx.x);
+
+  __shared__ int next_s[2];  // group this CTA takes next (written by thread 0, double-buffered over iterations)
+  int it = 0;
+  for (int grp = blockIdx.x; grp < ngroups; ++it) {
+    const size_t col = (size_t)grp * LINES + line;
+    const size_t e0 = ((size_t)t * nx + col) * 2 + c;  // element (row t, column col, component c)
+    // the next group is requested now and published before the last barrier of this iteration (latency hidden)
+    int nxt_req = 0;
+    if (tid == 0) nxt_req = sched_next(a.sched);
+    cp_async_wait_all();
+#pragma unroll
+    for (int n = 0; n < 16; ++n) v[n] = St::cv(stg[n * NTHR + tid]);
+    __syncthreads();  // every thread has taken its staged values: the buffers may be overwritten
+    int nxt_grp = ngroups;
 
     line_fft_fwd<NY>(buf, twS, t, c, v);
 
@@ -91,11 +111,21 @@ pass_y_kernel(const PassYArgs a) {
           double2 f = SM::EY_SMEM ? ey[pos] : __ldg(ey + pos + late_zero(v[g * P::RL + s].re));
           v[g * P::RL + s] = cmul(v[g * P::RL + s], mk(f.x, f.y));
         }
-      line_fft_inv<NY>(buf, twS, t, c, v);
+      // after the last read of the line buffers the next group's transfer starts under the last butterflies
+      auto hook = [&]() {
+        if (tid == 0) next_s[it & 1] = nxt_req;
+        __syncthreads();
+        nxt_grp = next_s[it & 1];
+        if (nxt_grp < ngroups) issue_loads(nxt_grp);
+      };
+      line_fft_inv<NY>(buf, twS, t, c, v, 0, hook);
 #pragma unroll
       for (int n = 0; n < 16; ++n) St::st(a.psi, e0 + n * estride, v[n]);
-      __syncthreads();  // the last exchange has been read by every warp before the next group writes
     } else {
+      if (tid == 0) next_s[it & 1] = nxt_req;
+      __syncthreads();
+      nxt_grp = next_s[it & 1];
+      if (nxt_grp < ngroups) issue_loads(nxt_grp);
       const double kx = a.Kx[(size_t)c * nx + col];
 #pragma unroll
       for (int g = 0; g < P::G; ++g)
@@ -104,9 +134,10 @@ pass_y_kernel(const PassYArgs a) {
           const cplx z = v[g * P::RL + s];
           e = fma(kx + a.Ky[(t + g * T) + (NY / P::RL) * s], fma(z.re, z.re, z.im * z.im), e);
         }
-      __syncthreads();
     }
+    grp = nxt_grp;
   }
+  if (tid == 0) sched_finish(a.sched);
 
   if (YMODE == YMODE_ENERGY) {
     __shared__ double red[32];
