@@ -7,6 +7,9 @@
 #include <new>
 #include <vector>
 
+#include <cuda.h>
+#include <cudaTypedefs.h>
+
 #include "../../include/spgpe.h"
 #include "internal.h"
 
@@ -30,6 +33,7 @@ struct spgpe_ctx {
   int tab_imag;
   bool tab_valid;
   double *partial, *scale, *target, *dout;
+  CUtensorMap tmap_psi, tmap_scratch;  // column-pass tensor maps of psi and of the energy scratch buffer
   int* sched;    // [4] work counters of the persistent kernels: row pass [0..1], column pass [2..3]
   double* fmax;  // [3] max |V|, |Omega|, |delta| (tier bounds of the row pass)
   int partial_cap;
@@ -78,6 +82,29 @@ static int cuda_fail(cudaError_t e) {
     cudaError_t e__ = (call);                     \
     if (e__ != cudaSuccess) return cuda_fail(e__); \
   } while (0)
+
+// Tensor map of a psi-shaped buffer for the column pass (pass_y.cuh): 2-D [ny rows][4 nx reals], box of
+// min(ny, 256) rows x 4 * lines reals.  The driver entry point is looked up at run time (no libcuda link).
+static cudaError_t make_col_tmap(const spgpe_ctx* h, void* base, int lines, CUtensorMap* out) {
+  static PFN_cuTensorMapEncodeTiled_v12000 encode = nullptr;
+  if (!encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q);
+    if (e != cudaSuccess) return e;
+    if (!fn || q != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
+    encode = (PFN_cuTensorMapEncodeTiled_v12000)fn;
+  }
+  const size_t rsz = (h->dt == SPGPE_C128) ? 8 : 4;
+  const cuuint64_t gdim[2] = {(cuuint64_t)h->nx * 4, (cuuint64_t)h->ny};
+  const cuuint64_t gstride[1] = {(cuuint64_t)h->nx * 4 * rsz};
+  const cuuint32_t box[2] = {(cuuint32_t)lines * 4, (cuuint32_t)(h->ny < 256 ? h->ny : 256)};
+  const cuuint32_t estr[2] = {1, 1};
+  CUresult r = encode(out, h->dt == SPGPE_C128 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
+                      base, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                      CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
 
 static bool size_ok(int n) { return n >= 64 && n <= 4096 && (n & (n - 1)) == 0; }
 
@@ -211,6 +238,7 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
     e = cudaMemcpy(h->Kx, Kx.data(), sizeof(double) * Kx.size(), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(h->Ky, Ky.data(), sizeof(double) * Ky.size(), cudaMemcpyHostToDevice);
   }
+  if (e == cudaSuccess) e = make_col_tmap(h, h->psi, plan_lines_y(ny), &h->tmap_psi);
   if (e != cudaSuccess) {
     spgpe_destroy(h);
     return cuda_fail(e);
@@ -329,7 +357,7 @@ extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
   xa.tau = 0.5 * dt; xa.hc = h->hc; xa.imag = imag; xa.want_norm = imag; xa.ny = h->ny; xa.fmax = h->fmax; xa.sched = h->sched;
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
-  ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx; ya.sched = h->sched + 2;
+  ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx; ya.sched = h->sched + 2; ya.tmap = h->tmap_psi;
   const double w = (h->Lx / h->nx) * (h->Ly / h->ny);
   if (!imag) {
     CK(dispatch_x(h, MODE_PRO, xa));
@@ -365,7 +393,10 @@ extern "C" int spgpe_norm(spgpe_handle h, double out[2]) {
 extern "C" int spgpe_energy(spgpe_handle h, double out[5]) {
   if (!h || !out) return SPGPE_ERR_INVALID_ARG;
   if (!h->ready) return SPGPE_ERR_NOT_READY;
-  if (!h->scratch) CK(cudaMalloc(&h->scratch, h->psi_bytes));
+  if (!h->scratch) {
+    CK(cudaMalloc(&h->scratch, h->psi_bytes));
+    CK(make_col_tmap(h, h->scratch, plan_lines_y(h->ny), &h->tmap_scratch));
+  }
   const double w = (h->Lx / h->nx) * (h->Ly / h->ny);
   const int nblk = 1024;
   h->launches += 4;
@@ -378,7 +409,7 @@ extern "C" int spgpe_energy(spgpe_handle h, double out[5]) {
   CK(dispatch_x(h, MODE_FWD, xa));
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
-  ya.psi = h->scratch; ya.tw = h->tw_y; ya.Kx = h->Kx; ya.Ky = h->Ky; ya.partial = h->partial; ya.nx = h->nx; ya.sched = h->sched + 2;
+  ya.psi = h->scratch; ya.tw = h->tw_y; ya.Kx = h->Kx; ya.Ky = h->Ky; ya.partial = h->partial; ya.nx = h->nx; ya.sched = h->sched + 2; ya.tmap = h->tmap_scratch;
   CK(dispatch_y(h, YMODE_ENERGY, ya));
   CK(aux_sum_partials(h->partial, h->ygrid, 1, w / ((double)h->nx * (double)h->ny), h->dout + 1,
                       h->stream));

@@ -23,6 +23,7 @@ SPGPE_DECL(4096)
 // host-side plan queries (tables.cu)
 int plan_tw_total(int n);                       // number of twiddle entries of length n
 void plan_fill_twiddles(int n, double2* host);  // exp(-2 pi i k lo / (16 M_j)) blocks, see common.cuh
+int plan_lines_y(int n);                        // columns per CTA of the column pass of length n
 int plan_freq_of_pos(int n, int pos);           // signed-less frequency index f in [0, n) stored at position pos
 
 // small kernels (aux.cu); all enqueue on s and return cudaGetLastError()

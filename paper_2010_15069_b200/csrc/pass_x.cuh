@@ -158,7 +158,7 @@ pass_x_kernel(const PassXArgs a) {
   typedef Store<DT> St;
   typedef typename St::real real;
   typedef typename St::elem elem;
-  extern __shared__ double2 smem[];
+  extern __shared__ __align__(128) double2 smem[];
   constexpr int NTHR = LINES * (NX / 8);
   constexpr int T = P::T;
   const int tid = threadIdx.x;

@@ -9,6 +9,8 @@
 //   YMODE_STEP   : psi^(k_x, y) -> F_y -> * ey(k_y) -> F_y^-1 -> psi^(k_x, y)            (in place)
 //   YMODE_ENERGY : psi^(k_x, y) -> F_y -> sum (Kx_c(k_x) + Ky(k_y)) |psi^|^2 -> partial[CTA]
 #pragma once
+#include <cuda.h>
+
 #include "line_fft.cuh"
 
 namespace spgpe {
@@ -24,6 +26,8 @@ struct PassYArgs {
   double* partial;      // [gridDim.x] sum over this CTA's columns (YMODE_ENERGY)
   int nx;
   int* sched;           // [2] device: work counter (common.cuh, sched_next)
+  // psi as a 2-D tensor [NY rows][4 nx reals], box = [min(NY, 256) rows][4 LINES reals]: the columns of a group
+  CUtensorMap tmap;
 };
 
 template <int NY, int LINES>
@@ -47,11 +51,11 @@ struct YSmem {
 // Persistent: CTA b handles the column groups b, b + gridDim.x, ...
 template <int DT, int NY, int LINES, int YMODE>
 __global__ void __launch_bounds__(LINES * (NY / 8), (LINES * (NY / 8) <= 256) ? 2 : 1)
-pass_y_kernel(const PassYArgs a) {
+pass_y_kernel(const __grid_constant__ PassYArgs a) {
   typedef Plan<NY> P;
   typedef Store<DT> St;
   typedef YSmem<NY, LINES> SM;
-  extern __shared__ double2 smem[];
+  extern __shared__ __align__(128) double2 smem[];
   constexpr int T = P::T;
   constexpr int NTHR = LINES * (NY / 8);
   const int tid = threadIdx.x;
@@ -74,17 +78,27 @@ pass_y_kernel(const PassYArgs a) {
   double e = 0.0;
   cplx v[16];
 
-  // The columns of a group travel global -> shared memory asynchronously (cp.async into the line buffers while
-  // they are idle: slot (n, tid) holds register n of thread tid), issued one group ahead.
+  // The columns of a group travel global -> shared memory through TMA: NY / BR boxes of BR rows x (LINES columns x
+  // 2 components), landing densely ([row][line][c]) in the line buffers while these are idle, issued one group
+  // ahead by one thread; completion is signalled on an mbarrier (phase = iteration parity).
   typedef typename St::elem elem;
+  constexpr int BR = NY < 256 ? NY : 256;
+  constexpr unsigned TILE_BYTES = (unsigned)NY * LINES * 2 * (unsigned)sizeof(elem);
   elem* stg = reinterpret_cast<elem*>(smem);
-  auto issue_loads = [&](int grp) {
-    const size_t col = (size_t)grp * LINES + line;
-    const elem* src = reinterpret_cast<const elem*>(a.psi) + ((size_t)t * nx + col) * 2 + c;
+  __shared__ __align__(8) unsigned long long mbar;
+  auto issue_loads = [&](int grp) {  // thread 0 only
+    fence_proxy_async();
+    mbar_expect_tx(&mbar, TILE_BYTES);
 #pragma unroll
-    for (int n = 0; n < 16; ++n) cp_async_elem(stg + n * NTHR + tid, src + n * estride);
+    for (int b = 0; b < NY / BR; ++b)
+      tma_load_2d(stg + (size_t)b * BR * LINES * 2, &a.tmap, grp * LINES * 4, b * BR, &mbar);
   };
-  if ((int)blockIdx.x < ngroups) issue_loads(blockIdx.x);
+  if (tid == 0) {
+    mbar_init(&mbar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if ((int)blockIdx.x < ngroups) issue_loads(blockIdx.x);
+  }
+  __syncthreads();
 
   __shared__ int next_s[2];  // group this CTA takes next (written by thread 0, double-buffered over iterations)
   int it = 0;
@@ -94,9 +108,9 @@ pass_y_kernel(const PassYArgs a) {
     // the next group is requested now and published before the last barrier of this iteration (latency hidden)
     int nxt_req = 0;
     if (tid == 0) nxt_req = sched_next(a.sched);
-    cp_async_wait_all();
+    mbar_wait(&mbar, it & 1);
 #pragma unroll
-    for (int n = 0; n < 16; ++n) v[n] = St::cv(stg[n * NTHR + tid]);
+    for (int n = 0; n < 16; ++n) v[n] = St::cv(stg[((t + n * T) * LINES + line) * 2 + c]);
     __syncthreads();  // every thread has taken its staged values: the buffers may be overwritten
     int nxt_grp = ngroups;
 
@@ -116,7 +130,7 @@ pass_y_kernel(const PassYArgs a) {
         if (tid == 0) next_s[it & 1] = nxt_req;
         __syncthreads();
         nxt_grp = next_s[it & 1];
-        if (nxt_grp < ngroups) issue_loads(nxt_grp);
+        if (tid == 0 && nxt_grp < ngroups) issue_loads(nxt_grp);
       };
       line_fft_inv<NY>(buf, twS, t, c, v, 0, hook);
 #pragma unroll
@@ -125,7 +139,7 @@ pass_y_kernel(const PassYArgs a) {
       if (tid == 0) next_s[it & 1] = nxt_req;
       __syncthreads();
       nxt_grp = next_s[it & 1];
-      if (nxt_grp < ngroups) issue_loads(nxt_grp);
+      if (tid == 0 && nxt_grp < ngroups) issue_loads(nxt_grp);
       const double kx = a.Kx[(size_t)c * nx + col];
 #pragma unroll
       for (int g = 0; g < P::G; ++g)

@@ -24,6 +24,8 @@ PlanInfo plan_info(int n) {
 }  // namespace
 
 
+int plan_lines_y(int n) { return plan_info(n).lines_y; }
+
 int plan_tw_total(int n) {
   PlanInfo p = plan_info(n);
   int total = 0;
