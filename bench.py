@@ -42,6 +42,19 @@ WORKLOADS = {
 }
 
 
+def read_traffic(workload: str, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full summary, or None."""
+    path = os.path.join(ROOT, "profiles", "r1_traffic.json")
+    try:
+        with open(path) as f:
+            d = json.load(f)
+        if d.get("workload") == workload:
+            return d["kernels"][kernel]["bytes_per_launch"]
+    except Exception:
+        pass
+    return None
+
+
 def read_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -131,6 +144,20 @@ def oracle_sample(w_cfg: int, dtype: str, budget_s: float, steps: int):
     return n * n / sec, threads, what, sec
 
 
+def whole_job_value(points: int, steps: int, ms_local: float, world: int, group=None):
+    """(value, ms) of the replicas-only job: every rank steps its own copy; the job's time is the max over ranks
+    (all_reduce MAX on whatever backend the group has) and value = world * points * steps / time."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_local], dtype=torch.float64)
+    if world > 1:
+        if dist.get_backend(group) == "nccl":
+            t = t.cuda()
+        dist.all_reduce(t, op=dist.ReduceOp.MAX, group=group)
+    ms = float(t.item())
+    return world * points * steps / (ms * 1e-3), ms
+
+
 def run_reference(args, wname):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -218,10 +245,7 @@ def run_ours(args, wname):
             fn()
             e1.record(stream)
         barrier()
-        ms = torch.tensor([e0.elapsed_time(e1)], device="cuda", dtype=torch.float64)
-        if world > 1:
-            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-        return float(ms.item())
+        return whole_job_value(P, K, e0.elapsed_time(e1), world)[1]
 
     sampler = ClockSampler(local)
     # ---- device-resident throughput --------------------------------------------------------------------
@@ -285,7 +309,8 @@ def run_ours(args, wname):
             "step_roofline_frac": step_bytes / (ms / K * 1e-3) / 1e9 / peak,
             "roofline": {"bound": "hbm", "kernel": ["pass_x_kernel (row pass)", "pass_y_kernel (column pass)"][dom],
                          "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None, "peak_source": peak_src,
+                         "traffic": read_traffic(w.name, ["pass_x_kernel", "pass_y_kernel"][dom]),
+                         "algorithmic_bytes": bytes_pt[dom] * P, "peak_source": peak_src,
                          "avg_launch_us": {"row_pass": 1e3 * avg[0], "column_pass": 1e3 * avg[1]},
                          "launches_timed": kcnt, "bytes_per_point": bytes_pt},
             "e2e": {"value": world * P * K / e2e_s, "unit": UNIT,

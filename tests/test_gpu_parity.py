@@ -194,3 +194,53 @@ def test_workload_configs_proxy(sp, cfg, n, steps):
         e_ref = orc.energy(ref, w.V, w.Omega, w.delta, p)
         e_got = sp.spgpe_energy(h)
         assert np.abs(e_got - e_ref).max() < TOL_E * np.abs(e_ref).max()
+
+
+# ---- full sizes of BASELINE.json, in the launch configuration bench.py times (persistent kernels, all SMs) ----
+@pytest.mark.parametrize("cfg,dtype,steps", [(4, "c128", 6), (4, "c64", 6), (3, "c128", 4)])
+def test_full_size_configs_few_steps(sp, cfg, dtype, steps):
+    """Configs 3 and 4 at their full grids (1024^2 imaginary time, 2048^2 real time): every element of psi after a
+    few steps against the oracle, plus norms and (complex128) the energy."""
+    orc.set_threads(orc.max_threads())
+    w = wl.make_workload(cfg, dtype=dtype)
+    h = sp.from_workload(w)
+    p = orc.params_of(w)
+    cnt, dt, imag = w.schedule[0]
+    sp.spgpe_step(h, steps, dt, imag)
+    got = sp.spgpe_get_psi_host(h)
+    ref = orc.step(w.psi0, w.V, w.Omega, w.delta, p, steps, dt, imag)
+    assert rel_l2(got, ref) < (TOL_C64 if dtype == "c64" else TOL_C128)
+    np.testing.assert_allclose(sp.spgpe_norm(h), orc.norm(ref, p), rtol=1e-6 if dtype == "c64" else 1e-12)
+    if dtype == "c128":
+        e_ref = orc.energy(ref, w.V, w.Omega, w.delta, p)
+        e_got = sp.spgpe_energy(h)
+        assert np.abs(e_got - e_ref).max() < TOL_E * np.abs(e_ref).max()
+
+
+def test_full_size_invariants_config4(sp):
+    """Properties that hold at any size: real time conserves both norms to rounding and the
+    energy oscillates within a small band; checked over 300 steps of config 4 at 2048^2."""
+    w = wl.make_workload(4)
+    h = sp.from_workload(w)
+    cnt, dt, imag = w.schedule[0]
+    n0, e0 = sp.spgpe_norm(h), sp.spgpe_energy(h)
+    sp.spgpe_step(h, 300, dt, 0)
+    n1, e1 = sp.spgpe_norm(h), sp.spgpe_energy(h)
+    assert abs(n1.sum() - n0.sum()) < 1e-11 * n0.sum()
+    # the split step conserves a modified energy: E itself moves by O(dt^2) times the (noise-dominated) kinetic scale
+    assert abs(e1[0] - e0[0]) < 1e-3 * abs(e0[0])
+    # step(n, dt) then step(n, -dt) returns the input when all g are equal (SURVEY.md 8(c), reversibility)
+    sp.spgpe_step(h, 300, -dt, 0)
+    back = sp.spgpe_get_psi_host(h)
+    assert rel_l2(back, w.psi0) < 1e-11
+
+
+def test_general_tier_rows_match_oracle(sp):
+    """Rows whose bounds leave the series tiers (large V tau, large |b| tau) next to rows that stay inside them."""
+    psi, V, Om, De, p, _ = random_problem(512, 128, seed=77)
+    V = V * np.where(np.arange(128)[:, None] % 3 == 0, 400.0, 1.0)
+    Om = Om * np.where(np.arange(128)[:, None] % 5 == 0, 300.0, 1.0)
+    h = make_solver(sp, psi, V, Om, De, p)
+    sp.spgpe_step(h, 3, 4e-3, 0)
+    ref = orc.step(psi, V, Om, De, p, 3, 4e-3, 0)
+    assert rel_l2(sp.spgpe_get_psi_host(h), ref) < TOL_C128
