@@ -134,6 +134,18 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const void* tmap, in
       : "memory");
 }
 
+// ---- programmatic dependent launch ----------------------------------------------------------------------------
+// The pass kernels are launched with programmatic stream serialization: a kernel may become resident while its
+// predecessor drains, runs its prologue (table copies, barrier set-up) and then waits here for the predecessor's
+// memory to be complete before it touches psi or the work counters.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// cooperative copy of n double2 entries global -> shared memory with cp.async (no register round trip)
+__device__ __forceinline__ void copy_table_async(double2* dst, const double2* src, int n, int tid, int nthreads) {
+  for (int i = tid; i < n; i += nthreads) cp_async16(dst + i, src + i);
+}
+
 // ---- dynamic work distribution of the persistent pass kernels -------------------------------------------------
 // sched[0] = number of groups handed out beyond the first gridDim.x, sched[1] = CTAs that have finished.  CTA b
 // starts with group b and then takes gridDim.x + atomicAdd(sched[0], 1), so that fast SMs take more groups than

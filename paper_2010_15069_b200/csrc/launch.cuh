@@ -28,6 +28,23 @@ cudaError_t resident_ctas(K kernel, int threads, size_t smem, int* out) {
   return cudaSuccess;
 }
 
+// launch with programmatic stream serialization (common.cuh, pdl_wait): the kernel may start its prologue while
+// the previous kernel on the stream drains
+template <typename K, typename A>
+cudaError_t launch_pdl(K kernel, int grid, int threads, size_t smem, cudaStream_t s, const A& args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3((unsigned)threads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, args);
+}
+
 // grid_out: number of CTAs launched (= rows of PassXArgs::partial written by MODE_EPI)
 template <int DT, int N, int MODE>
 cudaError_t launch_x(const PassXArgs& a, int ny, cudaStream_t s, int* grid_out) {
@@ -44,8 +61,7 @@ cudaError_t launch_x(const PassXArgs& a, int ny, cudaStream_t s, int* grid_out) 
   const int groups = ny / L;
   const int grid = groups < resident ? groups : resident;
   *grid_out = grid;
-  k<<<grid, L * (N / 8), smem, s>>>(a);
-  return cudaGetLastError();
+  return launch_pdl(k, grid, L * (N / 8), smem, s, a);
 }
 
 template <int DT, int N, int YMODE>
@@ -63,8 +79,7 @@ cudaError_t launch_y(const PassYArgs& a, cudaStream_t s, int* grid_out) {
   const int groups = a.nx / L;
   const int grid = groups < resident ? groups : resident;
   *grid_out = grid;
-  k<<<grid, L * (N / 8), smem, s>>>(a);
-  return cudaGetLastError();
+  return launch_pdl(k, grid, L * (N / 8), smem, s, a);
 }
 
 #define SPGPE_DEFINE_LAUNCHERS(N_)                                                               \

@@ -173,8 +173,9 @@ pass_x_kernel(const PassXArgs a) {
   cplx v[16];
   // twiddle table of NX behind the line buffers, copied once per (persistent) CTA
   double2* twS = smem + XSmem<NX, LINES>::EBUF;
-  for (int i = tid; i < tw_total<NX>(); i += LINES * (NX / 8)) twS[i] = a.tw[i];
-  __syncthreads();
+  pdl_launch_dependents();
+  copy_table_async(twS, a.tw, tw_total<NX>(), tid, NTHR);  // completes with the first cp_async_wait_all below
+  pdl_wait();
 
   // The psi rows of a group travel global -> shared memory asynchronously (cp.async into the line buffers, which
   // are idle at that time: slot (n, tid) holds register n of thread tid), issued one group ahead so that the

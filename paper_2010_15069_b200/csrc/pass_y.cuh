@@ -65,13 +65,13 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
   double2* buf = smem + (size_t)line * (YLayout<NY, LINES>::LINE_PTS * 2);
   double2* twS = smem + SM::EBUF;
   const double2* ey = a.eyk;
-  for (int i = tid; i < SM::TW; i += NTHR) twS[i] = a.tw[i];
+  pdl_launch_dependents();
+  copy_table_async(twS, a.tw, SM::TW, tid, NTHR);
   if (YMODE == YMODE_STEP && SM::EY_SMEM) {
     double2* eyS = twS + SM::TW;
-    for (int i = tid; i < NY; i += NTHR) eyS[i] = a.eyk[i];
+    copy_table_async(eyS, a.eyk, NY, tid, NTHR);
     ey = eyS;
   }
-  __syncthreads();
   const size_t nx = (size_t)a.nx;
   const int ngroups = a.nx / LINES;
   const size_t estride = (size_t)T * nx * 2;  // rows of one thread are T*nx points apart
@@ -96,9 +96,11 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
   if (tid == 0) {
     mbar_init(&mbar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    if ((int)blockIdx.x < ngroups) issue_loads(blockIdx.x);
   }
-  __syncthreads();
+  pdl_wait();  // psi, the phase table and the work counter belong to the preceding kernels
+  if (tid == 0 && (int)blockIdx.x < ngroups) issue_loads(blockIdx.x);
+  cp_async_wait_all();
+  __syncthreads();  // tables and the barrier are visible to every thread
 
   __shared__ int next_s[2];  // group this CTA takes next (written by thread 0, double-buffered over iterations)
   int it = 0;
