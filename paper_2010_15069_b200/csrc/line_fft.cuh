@@ -146,26 +146,45 @@ __device__ __forceinline__ void twiddle(const double2* tw, int t, cplx* v, int f
   }
 }
 
+// Synchronisation policy of a line transform.  sync(): barrier over the threads that share the line buffers;
+// acquire()/release(): bracket every exchange (the shared-memory stores, the barrier and the loads after it).
+// CtaSync: the whole CTA works on the same lines, no bracket.  GroupSync (pass_x.cuh): two thread groups of one
+// CTA work on different lines and take turns at their exchanges.
+struct CtaSync {
+  __device__ __forceinline__ void sync() const { __syncthreads(); }
+  __device__ __forceinline__ void acquire() const {}
+  __device__ __forceinline__ void release() const {}
+};
+template <int N, typename Sy>
+__device__ __forceinline__ void sync_last_p(const Sy& sy) {
+  if (Plan<N>::NS == 3) __syncwarp();
+  else sy.sync();
+}
+
 // one forward radix-16 stage J followed by the exchange into stage J+1's (or the last stage's) registers
-template <int N, int J>
-__device__ __forceinline__ void fwd_stages(double2* buf, const double2* tw, int t, int c, cplx* v, int flip) {
+template <int N, int J, typename Sy>
+__device__ __forceinline__ void fwd_stages(double2* buf, const double2* tw, int t, int c, cplx* v, int flip,
+                                           const Sy& sy) {
   if constexpr (J < Plan<N>::NS) {
     dft16<-1>(v);
     twiddle<N, J, -1>(tw, t, v, flip);
+    sy.acquire();
     sts_stage<N, J>(buf, t, c, v);
     if constexpr (J + 1 < Plan<N>::NS) {
-      __syncthreads();
+      sy.sync();
       lds_stage<N, J + 1>(buf, t, c, v);
     } else {
-      sync_last<N>();
+      sync_last_p<N>(sy);
       lds_last<N>(buf, t, c, v);
     }
-    fwd_stages<N, J + 1>(buf, tw, t, c, v, flip);
+    sy.release();
+    fwd_stages<N, J + 1>(buf, tw, t, c, v, flip, sy);
   }
 }
-template <int N>
-__device__ __forceinline__ void line_fft_fwd(double2* buf, const double2* tw, int t, int c, cplx* v, int flip = 0) {
-  fwd_stages<N, 1>(buf, tw, t, c, v, flip);
+template <int N, typename Sy = CtaSync>
+__device__ __forceinline__ void line_fft_fwd(double2* buf, const double2* tw, int t, int c, cplx* v, int flip = 0,
+                                             const Sy& sy = Sy()) {
+  fwd_stages<N, 1>(buf, tw, t, c, v, flip, sy);
   dft_last<-1, Plan<N>::RL>(v);
 }
 
@@ -174,29 +193,31 @@ struct NoHook {
 };
 // hook() runs right after the last read of the line buffer (the loads of stage 1): from there on the buffer is
 // free as soon as every warp has passed that point
-template <int N, int J, typename Hook>
+template <int N, int J, typename Hook, typename Sy>
 __device__ __forceinline__ void inv_stages(double2* buf, const double2* tw, int t, int c, cplx* v, int flip,
-                                           const Hook& hook) {
+                                           const Hook& hook, const Sy& sy) {
   if constexpr (J >= 1) {
+    sy.acquire();
     if constexpr (J + 1 < Plan<N>::NS) {
       sts_stage<N, J + 1>(buf, t, c, v);
-      __syncthreads();
+      sy.sync();
     } else {
       sts_last<N>(buf, t, c, v);
-      sync_last<N>();
+      sync_last_p<N>(sy);
     }
     lds_stage<N, J>(buf, t, c, v);
+    sy.release();
     if constexpr (J == 1) hook();
     twiddle<N, J, +1>(tw, t, v, flip);
     dft16<+1>(v);
-    inv_stages<N, J - 1>(buf, tw, t, c, v, flip, hook);
+    inv_stages<N, J - 1>(buf, tw, t, c, v, flip, hook, sy);
   }
 }
-template <int N, typename Hook = NoHook>
+template <int N, typename Hook = NoHook, typename Sy = CtaSync>
 __device__ __forceinline__ void line_fft_inv(double2* buf, const double2* tw, int t, int c, cplx* v, int flip = 0,
-                                             const Hook& hook = Hook()) {
+                                             const Hook& hook = Hook(), const Sy& sy = Sy()) {
   dft_last<+1, Plan<N>::RL>(v);
-  inv_stages<N, Plan<N>::NS - 1>(buf, tw, t, c, v, flip, hook);
+  inv_stages<N, Plan<N>::NS - 1>(buf, tw, t, c, v, flip, hook, sy);
 }
 
 }  // namespace spgpe

@@ -235,7 +235,7 @@ pass_x_kernel(const PassXArgs a) {
 #pragma unroll
       for (int n = 0; n < 16; ++n) St::st(a.dst, (rowbase + t + ((n + 8 * c) & 15) * T) * 2 + c, v[n]);
     } else {
-      fwd_stages<NX, 1>(buf, twS, t, c, v, flip);
+      fwd_stages<NX, 1>(buf, twS, t, c, v, flip, CtaSync());
       if (tid == 0) next_s[it & 1] = nxt_req;
       __syncthreads();  // the last exchange has been read by every warp: the line buffers are free
       nxt_grp = next_s[it & 1];
