@@ -136,6 +136,7 @@ def oracle_sample(w_cfg: int, dtype: str, budget_s: float, steps: int):
         if n >= full or 4.2 * sec * steps > budget_s:  # the next size costs ~4.2x
             break
         n *= 2
+    steps = int(min(200, max(steps, 12.0 / max(sec, 1e-3))))  # about 12 s of CPU work
     t0 = time.perf_counter()
     orc.step(w.psi0, w.V, w.Omega, w.delta, p, steps, dt, imag)
     sec = (time.perf_counter() - t0) / steps
