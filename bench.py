@@ -38,7 +38,7 @@ UNIT = "grid-point-steps/s"
 # pass; the row pass also reads the fields in use (one real per point each)
 WORKLOADS = {
     "4": dict(cfg=4, dtype="c128"), "4c64": dict(cfg=4, dtype="c64"), "3": dict(cfg=3, dtype="c128"),
-    "2": dict(cfg=2, dtype="c128"), "1": dict(cfg=1, dtype="c128"),
+    "2": dict(cfg=2, dtype="c128"), "1": dict(cfg=1, dtype="c128"), "5": dict(cfg=5, dtype="c64"),
 }
 
 

@@ -47,7 +47,7 @@ enum { SPGPE_NORM_PER_COMPONENT = 0, SPGPE_NORM_TOTAL = 1 }; /* R-7 */
 enum {
   SPGPE_OK = 0,
   SPGPE_ERR_INVALID_ARG = -1, /* NULL handle/pointer, non-positive size, unknown enum */
-  SPGPE_ERR_UNSUPPORTED = -2, /* nx or ny not a power of two in [64, 4096] */
+  SPGPE_ERR_UNSUPPORTED = -2, /* nx or ny not a power of two in [64, 8192] */
   SPGPE_ERR_NOT_READY = -3,   /* step/norm/energy/get before set_psi */
   SPGPE_ERR_CUDA = -4,        /* a CUDA call failed; spgpe_last_cuda_error() gives its text */
   SPGPE_ERR_NO_DEVICE = -5    /* no CUDA device / not an sm_100 device */

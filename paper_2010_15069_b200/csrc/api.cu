@@ -17,6 +17,8 @@ using namespace spgpe;
 
 struct spgpe_ctx {
   int nx, ny;
+  int sx, sy;  // 2: the axis is transformed as two interleaved sub-lines of length mx / my (split.cu), else 1
+  int mx, my;  // line lengths of the pass kernels: nx / sx, ny / sy
   double Lx, Ly;
   spgpe_params p;
   cudaStream_t stream;
@@ -35,6 +37,8 @@ struct spgpe_ctx {
   double *partial, *scale, *target, *dout;
   CUtensorMap tmap_psi, tmap_scratch;  // column-pass tensor maps of psi and of the energy scratch buffer
   int* sched;    // [4] work counters of the persistent kernels: row pass [0..1], column pass [2..3]
+  double2 *ones, *wcx, *wcy;  // split axes: k_x table of ones for the row pass, join twiddles
+  int *fpx, *fpy;             // split axes: true frequency of a sub-transform position
   double* fmax;  // [3] max |V|, |Omega|, |delta| (tier bounds of the row pass)
   int partial_cap;
   bool ready;
@@ -96,9 +100,10 @@ static cudaError_t make_col_tmap(const spgpe_ctx* h, void* base, int lines, CUte
     encode = (PFN_cuTensorMapEncodeTiled_v12000)fn;
   }
   const size_t rsz = (h->dt == SPGPE_C128) ? 8 : 4;
-  const cuuint64_t gdim[2] = {(cuuint64_t)h->nx * 4, (cuuint64_t)h->ny};
-  const cuuint64_t gstride[1] = {(cuuint64_t)h->nx * 4 * rsz};
-  const cuuint32_t box[2] = {(cuuint32_t)lines * 4, (cuuint32_t)(h->ny < 256 ? h->ny : 256)};
+  // a split y axis is seen as my rows of sy * nx points: row r of that view holds the rows sy * r + p of the grid
+  const cuuint64_t gdim[2] = {(cuuint64_t)h->nx * h->sy * 4, (cuuint64_t)h->my};
+  const cuuint64_t gstride[1] = {(cuuint64_t)h->nx * h->sy * 4 * rsz};
+  const cuuint32_t box[2] = {(cuuint32_t)lines * 4, (cuuint32_t)(h->my < 256 ? h->my : 256)};
   const cuuint32_t estr[2] = {1, 1};
   CUresult r = encode(out, h->dt == SPGPE_C128 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
                       base, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -106,21 +111,29 @@ static cudaError_t make_col_tmap(const spgpe_ctx* h, void* base, int lines, CUte
   return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
-static bool size_ok(int n) { return n >= 64 && n <= 4096 && (n & (n - 1)) == 0; }
+static bool size_ok(int n) { return n >= 64 && n <= 8192 && (n & (n - 1)) == 0; }
+// an axis is split when it is longer than the longest line of the pass kernels (or, for tests, when
+// SPGPE_DEBUG_SPLIT_MIN asks for it)
+static int split_of(int n) {
+  int nmin = 8192;
+  if (const char* e = getenv("SPGPE_DEBUG_SPLIT_MIN")) { const int v = atoi(e); if (v >= 128) nmin = v; }
+  return n >= nmin ? 2 : 1;
+}
 
 static cudaError_t dispatch_x_raw(spgpe_ctx* h, int mode, const PassXArgs& a) {
-  switch (h->nx) {
-    case 64: return launch_pass_x_64(h->dt, mode, a, h->ny, h->stream, &h->xgrid);
-    case 128: return launch_pass_x_128(h->dt, mode, a, h->ny, h->stream, &h->xgrid);
-    case 256: return launch_pass_x_256(h->dt, mode, a, h->ny, h->stream, &h->xgrid);
-    case 512: return launch_pass_x_512(h->dt, mode, a, h->ny, h->stream, &h->xgrid);
-    case 1024: return launch_pass_x_1024(h->dt, mode, a, h->ny, h->stream, &h->xgrid);
-    case 2048: return launch_pass_x_2048(h->dt, mode, a, h->ny, h->stream, &h->xgrid);
-    default: return launch_pass_x_4096(h->dt, mode, a, h->ny, h->stream, &h->xgrid);
+  const int nl = h->ny * h->sx;  // lines
+  switch (h->mx) {
+    case 64: return launch_pass_x_64(h->dt, mode, a, nl, h->stream, &h->xgrid);
+    case 128: return launch_pass_x_128(h->dt, mode, a, nl, h->stream, &h->xgrid);
+    case 256: return launch_pass_x_256(h->dt, mode, a, nl, h->stream, &h->xgrid);
+    case 512: return launch_pass_x_512(h->dt, mode, a, nl, h->stream, &h->xgrid);
+    case 1024: return launch_pass_x_1024(h->dt, mode, a, nl, h->stream, &h->xgrid);
+    case 2048: return launch_pass_x_2048(h->dt, mode, a, nl, h->stream, &h->xgrid);
+    default: return launch_pass_x_4096(h->dt, mode, a, nl, h->stream, &h->xgrid);
   }
 }
 static cudaError_t dispatch_y_raw(spgpe_ctx* h, int ymode, const PassYArgs& a) {
-  switch (h->ny) {
+  switch (h->my) {
     case 64: return launch_pass_y_64(h->dt, ymode, a, h->stream, &h->ygrid);
     case 128: return launch_pass_y_128(h->dt, ymode, a, h->stream, &h->ygrid);
     case 256: return launch_pass_y_256(h->dt, ymode, a, h->stream, &h->ygrid);
@@ -153,15 +166,16 @@ static void fill_ktables(const spgpe_ctx* h, std::vector<double>& Kx, std::vecto
   const double two_pi = 6.283185307179586476925286766559;
   Kx.resize(2 * (size_t)h->nx);
   Ky.resize(h->ny);
+  // unsplit axis: entry pos belongs to the frequency stored at pos; split axis: entry f belongs to frequency f
   for (int pos = 0; pos < h->nx; ++pos) {
-    const int f = plan_freq_of_pos(h->nx, pos);
+    const int f = h->sx == 1 ? plan_freq_of_pos(h->nx, pos) : pos;
     const int mt = (f < h->nx / 2) ? f : f - h->nx;
     const double k = two_pi * (double)mt / h->Lx;
     Kx[pos] = 0.5 * (k + h->p.k_L) * (k + h->p.k_L);
     Kx[h->nx + pos] = 0.5 * (k - h->p.k_L) * (k - h->p.k_L);
   }
   for (int pos = 0; pos < h->ny; ++pos) {
-    const int f = plan_freq_of_pos(h->ny, pos);
+    const int f = h->sy == 1 ? plan_freq_of_pos(h->ny, pos) : pos;
     const int mt = (f < h->ny / 2) ? f : f - h->ny;
     const double k = two_pi * (double)mt / h->Ly;
     Ky[pos] = 0.5 * k * k;
@@ -185,6 +199,7 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
   if (!h) return SPGPE_ERR_INVALID_ARG;
   memset(h, 0, sizeof(*h));
   h->nx = nx; h->ny = ny; h->Lx = Lx; h->Ly = Ly; h->p = *p;
+  h->sx = split_of(nx); h->sy = split_of(ny); h->mx = nx / h->sx; h->my = ny / h->sy;
   h->stream = (cudaStream_t)cuda_stream;
   h->dt = p->dtype;
   h->points = (size_t)nx * ny;
@@ -208,7 +223,7 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
   alloc(&h->Vbuf, h->field_bytes);
   alloc(&h->Ombuf, h->field_bytes);
   alloc(&h->Debuf, h->field_bytes);
-  const int twx = plan_tw_total(nx), twy = plan_tw_total(ny);
+  const int twx = plan_tw_total(h->mx), twy = plan_tw_total(h->my);
   alloc((void**)&h->tw_x, sizeof(double2) * twx);
   alloc((void**)&h->tw_y, sizeof(double2) * twy);
   alloc((void**)&h->Kx, sizeof(double) * 2 * nx);
@@ -225,10 +240,10 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
   if (e == cudaSuccess) e = cudaMemset(h->fmax, 0, sizeof(double) * 3);
   if (e == cudaSuccess) {
     std::vector<double2> tw(twx > twy ? twx : twy);
-    plan_fill_twiddles(nx, tw.data());
+    plan_fill_twiddles(h->mx, tw.data());
     e = cudaMemcpy(h->tw_x, tw.data(), sizeof(double2) * twx, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) {
-      plan_fill_twiddles(ny, tw.data());
+      plan_fill_twiddles(h->my, tw.data());
       e = cudaMemcpy(h->tw_y, tw.data(), sizeof(double2) * twy, cudaMemcpyHostToDevice);
     }
   }
@@ -238,7 +253,31 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
     e = cudaMemcpy(h->Kx, Kx.data(), sizeof(double) * Kx.size(), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(h->Ky, Ky.data(), sizeof(double) * Ky.size(), cudaMemcpyHostToDevice);
   }
-  if (e == cudaSuccess) e = make_col_tmap(h, h->psi, plan_lines_y(ny), &h->tmap_psi);
+  // join tables of the split axes
+  for (int ax = 0; ax < 2 && e == cudaSuccess; ++ax) {
+    const int sp = ax ? h->sy : h->sx, n = ax ? ny : nx, m = n / sp;
+    if (sp == 1) continue;
+    std::vector<int> fp(m);
+    std::vector<double2> wc(m);
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    for (int pos = 0; pos < m; ++pos) {
+      fp[pos] = plan_freq_of_pos(m, pos);
+      const long double ang = -two_pi * (long double)fp[pos] / (long double)n;
+      wc[pos] = make_double2((double)cosl(ang), (double)sinl(ang));
+    }
+    int** dfp = ax ? &h->fpy : &h->fpx;
+    double2** dwc = ax ? &h->wcy : &h->wcx;
+    alloc((void**)dfp, sizeof(int) * m);
+    alloc((void**)dwc, sizeof(double2) * m);
+    if (e == cudaSuccess) e = cudaMemcpy(*dfp, fp.data(), sizeof(int) * m, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(*dwc, wc.data(), sizeof(double2) * m, cudaMemcpyHostToDevice);
+    if (ax == 0) {
+      std::vector<double2> one(2 * (size_t)m, make_double2(1.0, 0.0));
+      alloc((void**)&h->ones, sizeof(double2) * one.size());
+      if (e == cudaSuccess) e = cudaMemcpy(h->ones, one.data(), sizeof(double2) * one.size(), cudaMemcpyHostToDevice);
+    }
+  }
+  if (e == cudaSuccess) e = make_col_tmap(h, h->psi, plan_lines_y(h->my), &h->tmap_psi);
   if (e != cudaSuccess) {
     spgpe_destroy(h);
     return cuda_fail(e);
@@ -251,7 +290,7 @@ extern "C" int spgpe_destroy(spgpe_handle h) {
   if (!h) return SPGPE_ERR_INVALID_ARG;
   cudaStreamSynchronize(h->stream);
   void* ptrs[] = {h->psi, h->scratch, h->Vbuf, h->Ombuf, h->Debuf, h->tw_x, h->tw_y, h->Kx, h->Ky,
-                  h->exk, h->eyk, h->partial, h->scale, h->target, h->dout, h->fmax, h->sched};
+                  h->exk, h->eyk, h->partial, h->scale, h->target, h->dout, h->fmax, h->sched, h->ones, h->wcx, h->wcy, h->fpx, h->fpy};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   if (h->prof_ev) {
@@ -343,6 +382,31 @@ static int ensure_tables(spgpe_handle h, double dt, int imag) {
   return SPGPE_OK;
 }
 
+static SplitArgs split_args(spgpe_ctx* h, void* psi) {
+  SplitArgs sa;
+  memset(&sa, 0, sizeof(sa));
+  sa.psi = psi; sa.nx = h->nx; sa.ny = h->ny; sa.fx = h->fpx; sa.fy = h->fpy; sa.wx = h->wcx; sa.wy = h->wcy;
+  sa.phx = h->exk; sa.phy = h->eyk; sa.Kx = h->Kx; sa.Ky = h->Ky; sa.partial = h->partial;
+  return sa;
+}
+
+// y transform, k-space phase, inverse y transform (between two row passes).  Unsplit: one column pass.  With a
+// split axis the join kernel (split.cu) applies the phases of the split axes on the joined spectrum.
+static cudaError_t kspace_part(spgpe_ctx* h, const PassYArgs& ya) {
+  cudaError_t e;
+  if (h->sx == 1 && h->sy == 1) return dispatch_y(h, YMODE_STEP, ya);
+  const SplitArgs sa = split_args(h, h->psi);
+  if (h->sy == 1) {  // only x is split: join along x (any y), then the ordinary column pass
+    h->launches++;
+    if ((e = launch_split(h->dt, sa, 2, 1, 0, 1184, h->stream)) != cudaSuccess) return e;
+    return dispatch_y(h, YMODE_STEP, ya);
+  }
+  if ((e = dispatch_y(h, YMODE_FWDONLY, ya)) != cudaSuccess) return e;
+  h->launches++;
+  if ((e = launch_split(h->dt, sa, h->sx, 2, 0, 1184, h->stream)) != cudaSuccess) return e;
+  return dispatch_y(h, YMODE_INVONLY, ya);
+}
+
 extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
   if (!h || n < 0 || !(dt == dt)) return SPGPE_ERR_INVALID_ARG;
   if (!h->ready) return SPGPE_ERR_NOT_READY;
@@ -353,23 +417,24 @@ extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
   PassXArgs xa;
   memset(&xa, 0, sizeof(xa));
   xa.src = h->psi; xa.dst = h->psi; xa.V = h->V; xa.Om = h->Om; xa.De = h->De;
-  xa.tw = h->tw_x; xa.exk = h->exk; xa.scale = nullptr; xa.partial = h->partial;
-  xa.tau = 0.5 * dt; xa.hc = h->hc; xa.imag = imag; xa.want_norm = imag; xa.ny = h->ny; xa.fmax = h->fmax; xa.sched = h->sched;
+  xa.tw = h->tw_x; xa.exk = h->sx == 1 ? h->exk : h->ones; xa.scale = nullptr; xa.partial = h->partial;
+  xa.tau = 0.5 * dt; xa.hc = h->hc; xa.imag = imag; xa.want_norm = imag; xa.ny = h->ny * h->sx; xa.xs = h->sx;
+  xa.fmax = h->fmax; xa.sched = h->sched;
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
-  ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx; ya.sched = h->sched + 2; ya.tmap = h->tmap_psi;
+  ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx * h->sy; ya.sched = h->sched + 2; ya.tmap = h->tmap_psi;
   const double w = (h->Lx / h->nx) * (h->Ly / h->ny);
   if (!imag) {
     CK(dispatch_x(h, MODE_PRO, xa));
     for (int s = 1; s <= n; ++s) {
-      CK(dispatch_y(h, YMODE_STEP, ya));
+      CK(kspace_part(h, ya));
       CK(dispatch_x(h, s < n ? MODE_MID : MODE_EPI, xa));
     }
   } else {
     for (int s = 0; s < n; ++s) {
       xa.scale = (s > 0) ? h->scale : nullptr;  // rescale of the previous step, applied at load
       CK(dispatch_x(h, MODE_PRO, xa));
-      CK(dispatch_y(h, YMODE_STEP, ya));
+      CK(kspace_part(h, ya));
       CK(dispatch_x(h, MODE_EPI, xa));
       h->launches++;
       CK(aux_norm_scale(h->partial, h->xgrid, w, h->target, h->p.norm_mode, h->scale, h->stream));
@@ -395,7 +460,7 @@ extern "C" int spgpe_energy(spgpe_handle h, double out[5]) {
   if (!h->ready) return SPGPE_ERR_NOT_READY;
   if (!h->scratch) {
     CK(cudaMalloc(&h->scratch, h->psi_bytes));
-    CK(make_col_tmap(h, h->scratch, plan_lines_y(h->ny), &h->tmap_scratch));
+    CK(make_col_tmap(h, h->scratch, plan_lines_y(h->my), &h->tmap_scratch));
   }
   const double w = (h->Lx / h->nx) * (h->Ly / h->ny);
   const int nblk = 1024;
@@ -405,13 +470,22 @@ extern "C" int spgpe_energy(spgpe_handle h, double out[5]) {
   CK(aux_sum_partials(h->partial, nblk, 3, w, h->dout + 2, h->stream));
   PassXArgs xa;
   memset(&xa, 0, sizeof(xa));
-  xa.src = h->psi; xa.dst = h->scratch; xa.tw = h->tw_x; xa.ny = h->ny; xa.sched = h->sched; xa.fmax = h->fmax;
+  xa.src = h->psi; xa.dst = h->scratch; xa.tw = h->tw_x; xa.ny = h->ny * h->sx; xa.xs = h->sx; xa.sched = h->sched; xa.fmax = h->fmax;
   CK(dispatch_x(h, MODE_FWD, xa));
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
-  ya.psi = h->scratch; ya.tw = h->tw_y; ya.Kx = h->Kx; ya.Ky = h->Ky; ya.partial = h->partial; ya.nx = h->nx; ya.sched = h->sched + 2; ya.tmap = h->tmap_scratch;
-  CK(dispatch_y(h, YMODE_ENERGY, ya));
-  CK(aux_sum_partials(h->partial, h->ygrid, 1, w / ((double)h->nx * (double)h->ny), h->dout + 1,
+  ya.psi = h->scratch; ya.tw = h->tw_y; ya.Kx = h->Kx; ya.Ky = h->Ky; ya.partial = h->partial; ya.nx = h->nx * h->sy; ya.sched = h->sched + 2; ya.tmap = h->tmap_scratch;
+  int kin_blocks;
+  if (h->sx == 1 && h->sy == 1) {
+    CK(dispatch_y(h, YMODE_ENERGY, ya));
+    kin_blocks = h->ygrid;
+  } else {  // full forward transform into the scratch buffer, then the join kernel sums K |psi^|^2
+    CK(dispatch_y(h, YMODE_FWDONLY, ya));
+    h->launches++;
+    kin_blocks = 1024;
+    CK(launch_split(h->dt, split_args(h, h->scratch), h->sx, h->sy, 1, kin_blocks, h->stream));
+  }
+  CK(aux_sum_partials(h->partial, kin_blocks, 1, w / ((double)h->nx * (double)h->ny), h->dout + 1,
                       h->stream));
   double tmp[5];
   CK(cudaMemcpyAsync(tmp + 1, h->dout + 1, 4 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
@@ -454,7 +528,7 @@ extern "C" const char* spgpe_strerror(int code) {
   switch (code) {
     case SPGPE_OK: return "ok";
     case SPGPE_ERR_INVALID_ARG: return "invalid argument";
-    case SPGPE_ERR_UNSUPPORTED: return "unsupported grid size (nx, ny must be powers of two in [64, 4096])";
+    case SPGPE_ERR_UNSUPPORTED: return "unsupported grid size (nx, ny must be powers of two in [64, 8192])";
     case SPGPE_ERR_NOT_READY: return "no order parameter set (call spgpe_set_psi first)";
     case SPGPE_ERR_CUDA: return "CUDA error (see spgpe_last_cuda_error)";
     case SPGPE_ERR_NO_DEVICE: return "no sm_100 CUDA device";

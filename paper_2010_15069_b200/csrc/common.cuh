@@ -96,6 +96,12 @@ __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gsrc) {
   const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
 }
+__device__ __forceinline__ void cp_async4(void* smem_dst, const void* gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_real(double* smem_dst, const double* gsrc) { cp_async8(smem_dst, gsrc); }
+__device__ __forceinline__ void cp_async_real(float* smem_dst, const float* gsrc) { cp_async4(smem_dst, gsrc); }
 __device__ __forceinline__ void cp_async_elem(double2* smem_dst, const double2* gsrc) { cp_async16(smem_dst, gsrc); }
 __device__ __forceinline__ void cp_async_elem(float2* smem_dst, const float2* gsrc) { cp_async8(smem_dst, gsrc); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }

@@ -20,6 +20,22 @@ SPGPE_DECL(2048)
 SPGPE_DECL(4096)
 #undef SPGPE_DECL
 
+// join of the two interleaved sub-transforms of an axis longer than 4096 (split.cu)
+struct SplitArgs {
+  void* psi;           // [ny][nx][2]
+  int nx, ny;          // full grid
+  const int* fx;       // [nx/2] true frequency (0..nx/2-1) of sub-transform position pos; split x axis only
+  const int* fy;       // [ny/2]
+  const double2* wx;   // [nx/2] exp(-2 pi i fx[pos] / nx)
+  const double2* wy;   // [ny/2]
+  const double2* phx;  // [2][nx] k_x phase by true frequency (split x axis only)
+  const double2* phy;  // [ny]    k_y phase by true frequency, 1/(nx ny) included (split y axis only)
+  const double* Kx;    // [2][nx] energy mode: by true frequency (split axis) or by stored position (unsplit)
+  const double* Ky;    // [ny]
+  double* partial;     // [gridDim.x] energy mode
+};
+cudaError_t launch_split(int dt, const SplitArgs& a, int sx, int sy, int energy, int nblk, cudaStream_t s);
+
 // host-side plan queries (tables.cu)
 int plan_tw_total(int n);                       // number of twiddle entries of length n
 void plan_fill_twiddles(int n, double2* host);  // exp(-2 pi i k lo / (16 M_j)) blocks, see common.cuh

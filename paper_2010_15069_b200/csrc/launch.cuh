@@ -100,11 +100,20 @@ cudaError_t launch_y(const PassYArgs& a, cudaStream_t s, int* grid_out) {
     }                                                                                            \
   }                                                                                              \
   cudaError_t launch_pass_y_##N_(int dt, int ymode, const PassYArgs& a, cudaStream_t s, int* g) { \
-    if (dt == 0)                                                                                 \
-      return ymode == YMODE_STEP ? launch_y<0, N_, YMODE_STEP>(a, s, g)                             \
-                                 : launch_y<0, N_, YMODE_ENERGY>(a, s, g);                          \
-    return ymode == YMODE_STEP ? launch_y<1, N_, YMODE_STEP>(a, s, g)                               \
-                               : launch_y<1, N_, YMODE_ENERGY>(a, s, g);                            \
+    if (dt == 0) {                                                                               \
+      switch (ymode) {                                                                           \
+        case YMODE_STEP: return launch_y<0, N_, YMODE_STEP>(a, s, g);                            \
+        case YMODE_ENERGY: return launch_y<0, N_, YMODE_ENERGY>(a, s, g);                        \
+        case YMODE_FWDONLY: return launch_y<0, N_, YMODE_FWDONLY>(a, s, g);                      \
+        default: return launch_y<0, N_, YMODE_INVONLY>(a, s, g);                                 \
+      }                                                                                          \
+    }                                                                                            \
+    switch (ymode) {                                                                             \
+      case YMODE_STEP: return launch_y<1, N_, YMODE_STEP>(a, s, g);                              \
+      case YMODE_ENERGY: return launch_y<1, N_, YMODE_ENERGY>(a, s, g);                          \
+      case YMODE_FWDONLY: return launch_y<1, N_, YMODE_FWDONLY>(a, s, g);                        \
+      default: return launch_y<1, N_, YMODE_INVONLY>(a, s, g);                                   \
+    }                                                                                            \
   }
 
 }  // namespace spgpe

@@ -32,7 +32,8 @@ struct PassXArgs {
   HalfCoef hc;
   int imag;
   int want_norm;
-  int ny;                // number of rows
+  int ny;                // number of lines (rows x xs)
+  int xs;                // 1: a line is a row; 2: a line is every second point of a row (split transform, api.cu)
   int* sched;            // [2] device: work counter (common.cuh, sched_next)
   const double* fmax;    // [3] device: max |V|, max |Omega|, max |delta| over the grid (tier bounds)
 };
@@ -43,12 +44,27 @@ __device__ __forceinline__ cplx shfl_xor_c(cplx a, int m) { return mk(shfl_xor_d
 // Copy the three field rows of this CTA's LINES rows into shared memory ([field][line][x], working precision),
 // 16 bytes per cp.async; a NULL field is filled with zeros.  Every thread of the CTA takes part.
 template <int DT, int NX, int LINES>
-__device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, size_t first_point, int tid) {
+__device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, size_t first_point, int first_line,
+                                             int tid) {
   typedef typename Store<DT>::real real;
   constexpr int FIELD_BYTES = LINES * NX * (int)sizeof(real);
   constexpr int NCH = FIELD_BYTES / 16;
   constexpr int NTHR = LINES * (NX / 8);
   const void* src[3] = {a.V, a.Om, a.De};
+  if (a.xs != 1) {  // strided lines: one cp.async per real
+    const int S = a.xs;
+#pragma unroll
+    for (int f = 0; f < 3; ++f) {
+      real* dst = reinterpret_cast<real*>(fbuf) + f * (LINES * NX);
+      const real* g = reinterpret_cast<const real*>(src[f]);
+      for (int k = tid; k < LINES * NX; k += NTHR) {
+        const int L = first_line + k / NX, pos = k % NX;
+        if (g != nullptr) cp_async_real(dst + k, g + (size_t)(L / S) * NX * S + (size_t)pos * S + (L % S));
+        else dst[k] = (real)0;
+      }
+    }
+    return;
+  }
 #pragma unroll
   for (int f = 0; f < 3; ++f) {
     char* dst = reinterpret_cast<char*>(fbuf) + f * FIELD_BYTES;
@@ -181,19 +197,23 @@ pass_x_kernel(const PassXArgs a) {
   // are idle at that time: slot (n, tid) holds register n of thread tid), issued one group ahead so that the
   // transfer runs under the tail of the previous group instead of stalling the CTA at the head of this one.
   elem* stg = reinterpret_cast<elem*>(smem);
+  // point index of position 0 of line L: lines are rows (xs = 1) or the even / odd points of a row (xs = 2)
+  const int S = a.xs;
+  auto line_base = [&](int L) { return (size_t)(L / S) * NX * S + (size_t)(L % S); };
   auto issue_loads = [&](int grp) {
-    const size_t rb = ((size_t)grp * LINES + line) * NX;
+    const size_t lb = line_base(grp * LINES + line);
     const elem* src = reinterpret_cast<const elem*>(a.src);
     if (MODE == MODE_PRO || MODE == MODE_FWD) {
 #pragma unroll
       for (int n = 0; n < 16; ++n)
-        cp_async_elem(stg + n * NTHR + tid, src + (rb + t + ((n + 8 * c) & 15) * T) * 2 + c);
+        cp_async_elem(stg + n * NTHR + tid, src + (lb + (size_t)(t + ((n + 8 * c) & 15) * T) * S) * 2 + c);
     } else {
 #pragma unroll
       for (int g = 0; g < P::G; ++g)
 #pragma unroll
         for (int s = 0; s < P::RL; ++s)
-          cp_async_elem(stg + (g * P::RL + s) * NTHR + tid, src + (rb + (t + g * T) + (NX / P::RL) * s) * 2 + c);
+          cp_async_elem(stg + (g * P::RL + s) * NTHR + tid,
+                        src + (lb + (size_t)((t + g * T) + (NX / P::RL) * s) * S) * 2 + c);
     }
   };
   if ((int)blockIdx.x < ngroups) issue_loads(blockIdx.x);
@@ -201,8 +221,8 @@ pass_x_kernel(const PassXArgs a) {
   __shared__ int next_s[2];  // group this CTA takes next (written by thread 0, double-buffered over iterations)
   int it = 0;
   for (int grp = blockIdx.x; grp < ngroups; ++it) {
-    const size_t first_point = (size_t)grp * LINES * NX;  // first point of the CTA's rows
-    const size_t rowbase = first_point + (size_t)line * NX;
+    const size_t first_point = (size_t)grp * LINES * NX;  // first point of the CTA's lines (xs = 1)
+    const size_t lbase = line_base(grp * LINES + line);
     // the next group is requested now and published before the last barrier of this iteration (latency hidden)
     int nxt_req = 0;
     if (tid == 0) nxt_req = sched_next(a.sched);
@@ -220,7 +240,7 @@ pass_x_kernel(const PassXArgs a) {
     if (MODE != MODE_FWD) {
       // the exchange buffer is idle during the real-space part: it holds the field rows meanwhile
       __syncthreads();
-      stage_fields<DT, NX, LINES>(smem, a, first_point, tid);
+      stage_fields<DT, NX, LINES>(smem, a, first_point, grp * LINES, tid);
       cp_async_wait_all();
       __syncthreads();
       real_space<DT, NX, LINES, MODE>(v, a, smem, line, t, c, lc, sm, so);
@@ -233,7 +253,7 @@ pass_x_kernel(const PassXArgs a) {
       nxt_grp = next_s[it & 1];
       if (nxt_grp < ngroups) issue_loads(nxt_grp);  // the line buffers are free after the real-space part
 #pragma unroll
-      for (int n = 0; n < 16; ++n) St::st(a.dst, (rowbase + t + ((n + 8 * c) & 15) * T) * 2 + c, v[n]);
+      for (int n = 0; n < 16; ++n) St::st(a.dst, (lbase + (size_t)(t + ((n + 8 * c) & 15) * T) * S) * 2 + c, v[n]);
     } else {
       fwd_stages<NX, 1>(buf, twS, t, c, v, flip, CtaSync());
       if (tid == 0) next_s[it & 1] = nxt_req;
@@ -253,10 +273,10 @@ pass_x_kernel(const PassXArgs a) {
             double2 e = __ldg(ex + off);
             o = cmul(o, mk(e.x, e.y));
           }
-          St::st(a.dst, (rowbase + t + off) * 2 + c, o);
+          St::st(a.dst, (lbase + (size_t)(t + off) * S) * 2 + c, o);
         }
     }
-    if (MODE != MODE_FWD && tid == 0 && nxt_grp < ngroups) {  // field rows of the next group: into L2
+    if (MODE != MODE_FWD && S == 1 && tid == 0 && nxt_grp < ngroups) {  // field rows of the next group: into L2
       const size_t nxt = (size_t)nxt_grp * LINES * NX;
       if (a.V) prefetch_l2_bulk(reinterpret_cast<const real*>(a.V) + nxt, LINES * NX * (unsigned)sizeof(real));
       if (a.Om) prefetch_l2_bulk(reinterpret_cast<const real*>(a.Om) + nxt, LINES * NX * (unsigned)sizeof(real));

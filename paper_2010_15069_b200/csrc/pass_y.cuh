@@ -8,6 +8,8 @@
 //
 //   YMODE_STEP   : psi^(k_x, y) -> F_y -> * ey(k_y) -> F_y^-1 -> psi^(k_x, y)            (in place)
 //   YMODE_ENERGY : psi^(k_x, y) -> F_y -> sum (Kx_c(k_x) + Ky(k_y)) |psi^|^2 -> partial[CTA]
+//   YMODE_FWDONLY: psi^(k_x, y) -> F_y -> psi^(k_x, k_y) in stored order          (split transforms, api.cu)
+//   YMODE_INVONLY: psi^(k_x, k_y) in stored order -> F_y^-1 -> psi^(k_x, y)
 #pragma once
 #include <cuda.h>
 
@@ -15,7 +17,7 @@
 
 namespace spgpe {
 
-enum { YMODE_STEP = 0, YMODE_ENERGY = 1 };
+enum { YMODE_STEP = 0, YMODE_ENERGY = 1, YMODE_FWDONLY = 2, YMODE_INVONLY = 3 };
 
 struct PassYArgs {
   void* psi;            // [NY][nx][2]
@@ -111,14 +113,23 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
     int nxt_req = 0;
     if (tid == 0) nxt_req = sched_next(a.sched);
     mbar_wait(&mbar, it & 1);
+    if (YMODE == YMODE_INVONLY) {
 #pragma unroll
-    for (int n = 0; n < 16; ++n) v[n] = St::cv(stg[((t + n * T) * LINES + line) * 2 + c]);
+      for (int g = 0; g < P::G; ++g)
+#pragma unroll
+        for (int s = 0; s < P::RL; ++s)
+          v[g * P::RL + s] = St::cv(stg[(((t + g * T) + (NY / P::RL) * s) * LINES + line) * 2 + c]);
+    } else {
+#pragma unroll
+      for (int n = 0; n < 16; ++n) v[n] = St::cv(stg[((t + n * T) * LINES + line) * 2 + c]);
+    }
     __syncthreads();  // every thread has taken its staged values: the buffers may be overwritten
     int nxt_grp = ngroups;
 
-    line_fft_fwd<NY>(buf, twS, t, c, v);
+    if (YMODE != YMODE_INVONLY) line_fft_fwd<NY>(buf, twS, t, c, v);
 
-    if (YMODE == YMODE_STEP) {
+    if (YMODE == YMODE_STEP || YMODE == YMODE_INVONLY) {
+      if (YMODE == YMODE_STEP) {
 #pragma unroll
       for (int g = 0; g < P::G; ++g)
 #pragma unroll
@@ -127,6 +138,7 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
           double2 f = SM::EY_SMEM ? ey[pos] : __ldg(ey + pos + late_zero(v[g * P::RL + s].re));
           v[g * P::RL + s] = cmul(v[g * P::RL + s], mk(f.x, f.y));
         }
+      }
       // after the last read of the line buffers the next group's transfer starts under the last butterflies
       auto hook = [&]() {
         if (tid == 0) next_s[it & 1] = nxt_req;
@@ -137,6 +149,18 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
       line_fft_inv<NY>(buf, twS, t, c, v, 0, hook);
 #pragma unroll
       for (int n = 0; n < 16; ++n) St::st(a.psi, e0 + n * estride, v[n]);
+    } else if (YMODE == YMODE_FWDONLY) {
+      if (tid == 0) next_s[it & 1] = nxt_req;
+      __syncthreads();
+      nxt_grp = next_s[it & 1];
+      if (tid == 0 && nxt_grp < ngroups) issue_loads(nxt_grp);
+#pragma unroll
+      for (int g = 0; g < P::G; ++g)
+#pragma unroll
+        for (int s = 0; s < P::RL; ++s) {
+          const size_t pos = (size_t)((t + g * T) + (NY / P::RL) * s);
+          St::st(a.psi, (pos * nx + col) * 2 + c, v[g * P::RL + s]);
+        }
     } else {
       if (tid == 0) next_s[it & 1] = nxt_req;
       __syncthreads();

@@ -1,0 +1,150 @@
+// split.cu -- line lengths above 4096 (one line no longer fits one CTA's registers and shared memory).
+//
+// An axis of length n = 2 m is transformed as two interleaved sub-lines of length m (even and odd samples) by the
+// ordinary pass kernels; this kernel supplies the radix-2 decimation-in-time step that joins them, applies the
+// k-space phase of the split axes on the joined spectrum and undoes the join:
+//   X[f]     = E[f] + w^f O[f],   X[f + m] = E[f] - w^f O[f],   w = exp(-2 pi i / n),  f = 0..m-1
+//   X <- phase * X                                              (on the split axes only)
+//   E'[f]    = X[f] + X[f + m],   O'[f]    = conj(w^f) (X[f] - X[f + m])          (unnormalised, like the passes)
+// E and O sit interleaved in memory: sub-line p of the x axis occupies the points x = 2 pos + p, sub-line p of the
+// y axis the rows y = 2 pos + p, pos = stored position of the sub-transform.  One thread owns the SX x SY block of
+// one (pos_x, pos_y) and both components, so the step is local and in place.
+// MODE_ENERGY instead accumulates sum (Kx_c + Ky) |X|^2 (spgpe_energy) and writes nothing back.
+#include "internal.h"
+
+namespace spgpe {
+
+template <int DT, int SX, int SY, bool ENERGY>
+__global__ void __launch_bounds__(256) split_kernel(const SplitArgs a) {
+  typedef Store<DT> St;
+  const int mx = a.nx / SX, my = a.ny / SY;
+  double esum = 0.0;
+  for (size_t b = (size_t)blockIdx.x * blockDim.x + threadIdx.x; b < (size_t)mx * my;
+       b += (size_t)gridDim.x * blockDim.x) {
+    const int px = (int)(b % mx), py = (int)(b / mx);
+    cplx u[SY][SX][2];
+#pragma unroll
+    for (int j = 0; j < SY; ++j)
+#pragma unroll
+      for (int i = 0; i < SX; ++i)
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+          u[j][i][c] = St::ld(a.psi, (((size_t)py * SY + j) * a.nx + (size_t)px * SX + i) * 2 + c);
+    // true frequencies of the block: f + ax m along a split axis; along an unsplit axis the stored position itself
+    // indexes the (stored-order) tables
+    const int fx = SX == 2 ? a.fx[px] : px, fy = SY == 2 ? a.fy[py] : py;
+    if (SX == 2) {
+      const double2 w = a.wx[px];
+#pragma unroll
+      for (int j = 0; j < SY; ++j)
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+          const cplx e = u[j][0][c], o = cmul(u[j][1][c], mk(w.x, w.y));
+          u[j][0][c] = e + o;
+          u[j][1][c] = e - o;
+        }
+    }
+    if (SY == 2) {
+      const double2 w = a.wy[py];
+#pragma unroll
+      for (int i = 0; i < SX; ++i)
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+          const cplx e = u[0][i][c], o = cmul(u[1][i][c], mk(w.x, w.y));
+          u[0][i][c] = e + o;
+          u[1][i][c] = e - o;
+        }
+    }
+    if (ENERGY) {
+#pragma unroll
+      for (int j = 0; j < SY; ++j)
+#pragma unroll
+        for (int i = 0; i < SX; ++i)
+#pragma unroll
+          for (int c = 0; c < 2; ++c) {
+            const double k = a.Kx[(size_t)c * a.nx + fx + i * mx] + a.Ky[fy + j * my];
+            esum = fma(k, fma(u[j][i][c].re, u[j][i][c].re, u[j][i][c].im * u[j][i][c].im), esum);
+          }
+      continue;
+    }
+    if (SX == 2) {
+#pragma unroll
+      for (int j = 0; j < SY; ++j)
+#pragma unroll
+        for (int i = 0; i < SX; ++i)
+#pragma unroll
+          for (int c = 0; c < 2; ++c) {
+            const double2 p = a.phx[(size_t)c * a.nx + fx + i * mx];
+            u[j][i][c] = cmul(u[j][i][c], mk(p.x, p.y));
+          }
+    }
+    if (SY == 2) {
+#pragma unroll
+      for (int j = 0; j < SY; ++j) {
+        const double2 p = a.phy[fy + j * my];
+#pragma unroll
+        for (int i = 0; i < SX; ++i)
+#pragma unroll
+          for (int c = 0; c < 2; ++c) u[j][i][c] = cmul(u[j][i][c], mk(p.x, p.y));
+      }
+    }
+    if (SY == 2) {
+      const double2 w = a.wy[py];
+#pragma unroll
+      for (int i = 0; i < SX; ++i)
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+          const cplx s = u[0][i][c] + u[1][i][c], d = u[0][i][c] - u[1][i][c];
+          u[0][i][c] = s;
+          u[1][i][c] = cmulc(d, mk(w.x, w.y));
+        }
+    }
+    if (SX == 2) {
+      const double2 w = a.wx[px];
+#pragma unroll
+      for (int j = 0; j < SY; ++j)
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+          const cplx s = u[j][0][c] + u[j][1][c], d = u[j][0][c] - u[j][1][c];
+          u[j][0][c] = s;
+          u[j][1][c] = cmulc(d, mk(w.x, w.y));
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < SY; ++j)
+#pragma unroll
+      for (int i = 0; i < SX; ++i)
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+          St::st(a.psi, (((size_t)py * SY + j) * a.nx + (size_t)px * SX + i) * 2 + c, u[j][i][c]);
+  }
+  if (ENERGY) {
+    __shared__ double red[8];
+#pragma unroll
+    for (int m = 16; m >= 1; m >>= 1) esum += __shfl_xor_sync(0xffffffffu, esum, m);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = esum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      double s = 0.0;
+      for (int i = 0; i < (int)(blockDim.x >> 5); ++i) s += red[i];
+      a.partial[blockIdx.x] = s;
+    }
+  }
+}
+
+template <int DT, bool ENERGY>
+static cudaError_t launch_split_dt(const SplitArgs& a, int sx, int sy, int nblk, cudaStream_t s) {
+  if (sx == 2 && sy == 2) split_kernel<DT, 2, 2, ENERGY><<<nblk, 256, 0, s>>>(a);
+  else if (sx == 2) split_kernel<DT, 2, 1, ENERGY><<<nblk, 256, 0, s>>>(a);
+  else if (sy == 2) split_kernel<DT, 1, 2, ENERGY><<<nblk, 256, 0, s>>>(a);
+  else split_kernel<DT, 1, 1, ENERGY><<<nblk, 256, 0, s>>>(a);
+  return cudaGetLastError();
+}
+
+// nblk CTAs of 256 threads; with energy != 0 partial[nblk] receives the per-CTA sums
+cudaError_t launch_split(int dt, const SplitArgs& a, int sx, int sy, int energy, int nblk, cudaStream_t s) {
+  if (dt == 0) return energy ? launch_split_dt<0, true>(a, sx, sy, nblk, s) : launch_split_dt<0, false>(a, sx, sy, nblk, s);
+  return energy ? launch_split_dt<1, true>(a, sx, sy, nblk, s) : launch_split_dt<1, false>(a, sx, sy, nblk, s);
+}
+
+}  // namespace spgpe

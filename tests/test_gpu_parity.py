@@ -244,3 +244,43 @@ def test_general_tier_rows_match_oracle(sp):
     sp.spgpe_step(h, 3, 4e-3, 0)
     ref = orc.step(psi, V, Om, De, p, 3, 4e-3, 0)
     assert rel_l2(sp.spgpe_get_psi_host(h), ref) < TOL_C128
+
+
+# ---- split axes (line lengths above 4096 are transformed as two interleaved half-length lines, split.cu) ----
+@pytest.mark.parametrize("nx,ny", [(128, 64), (64, 128), (128, 128), (256, 512), (1024, 128)])
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_split_axes_small_sizes(sp, monkeypatch, nx, ny, dtype):
+    """The split path is forced at small sizes (SPGPE_DEBUG_SPLIT_MIN) so that the oracle can check it quickly:
+    x only, y only, both; real and imaginary time; norm and energy."""
+    monkeypatch.setenv("SPGPE_DEBUG_SPLIT_MIN", str(min(128, max(nx, ny))) if max(nx, ny) < 256 else "256")
+    psi, V, Om, De, p, _ = random_problem(nx, ny, seed=nx + 3 * ny)
+    if dtype == "c64":
+        psi = psi.astype(np.complex64).astype(np.complex128)
+        V, Om, De = (a.astype(np.float32).astype(np.float64) for a in (V, Om, De))
+    tol = TOL_C64 if dtype == "c64" else TOL_C128
+    h = make_solver(sp, psi, V, Om, De, p, dtype=dtype)
+    sp.spgpe_step(h, 3, 2e-3, 0)
+    ref = orc.step(psi, V, Om, De, p, 3, 2e-3, 0)
+    assert rel_l2(sp.spgpe_get_psi_host(h), ref) < tol
+    if dtype == "c128":
+        e_ref = orc.energy(ref, V, Om, De, p)
+        assert np.abs(sp.spgpe_energy(h) - e_ref).max() < TOL_E * np.abs(e_ref).max()
+    sp.spgpe_step(h, 2, 1e-3, 1)
+    ref2 = orc.step(ref, V, Om, De, p, 2, 1e-3, 1, targets=orc.norm(psi, p))
+    assert rel_l2(sp.spgpe_get_psi_host(h), ref2) < tol
+
+
+@pytest.mark.slow
+def test_config5_full_size_one_step(sp):
+    """Config 5 (8192 x 8192, complex64 storage): one real-time step against the oracle on every element."""
+    if not os.environ.get("SPGPE_FULL"):
+        pytest.skip("set SPGPE_FULL=1 (builds 1 GiB arrays, oracle takes minutes)")
+    orc.set_threads(orc.max_threads())
+    w = wl.make_workload(5)
+    h = sp.from_workload(w)
+    p = orc.params_of(w)
+    cnt, dt, imag = w.schedule[0]
+    sp.spgpe_step(h, 1, dt, imag)
+    got = sp.spgpe_get_psi_host(h)
+    ref = orc.step(w.psi0, w.V, w.Omega, w.delta, p, 1, dt, imag)
+    assert rel_l2(got, ref) < TOL_C64
