@@ -28,6 +28,9 @@ cudaError_t resident_ctas(K kernel, int threads, size_t smem, int* out) {
   return cudaSuccess;
 }
 
+template <int DT, int N, int MODE>
+cudaError_t launch_x(const PassXArgs& a, int ny, cudaStream_t s, int* grid_out);
+
 // launch with programmatic stream serialization (common.cuh, pdl_wait): the kernel may start its prologue while
 // the previous kernel on the stream drains
 template <typename K, typename A>
@@ -46,10 +49,10 @@ cudaError_t launch_pdl(K kernel, int grid, int threads, size_t smem, cudaStream_
 }
 
 // grid_out: number of CTAs launched (= rows of PassXArgs::partial written by MODE_EPI)
-template <int DT, int N, int MODE>
-cudaError_t launch_x(const PassXArgs& a, int ny, cudaStream_t s, int* grid_out) {
+template <int DT, int N, int MODE, int XS>
+cudaError_t launch_x_xs(const PassXArgs& a, int ny, cudaStream_t s, int* grid_out) {
   constexpr int L = Lines<N>::X;
-  auto k = pass_x_kernel<DT, N, L, MODE>;
+  auto k = pass_x_kernel<DT, N, L, MODE, XS>;
   constexpr size_t smem = XSmem<N, L>::BYTES;
   static int resident = 0;
   if (resident == 0) {
@@ -62,6 +65,11 @@ cudaError_t launch_x(const PassXArgs& a, int ny, cudaStream_t s, int* grid_out) 
   const int grid = groups < resident ? groups : resident;
   *grid_out = grid;
   return launch_pdl(k, grid, L * (N / 8), smem, s, a);
+}
+
+template <int DT, int N, int MODE>
+cudaError_t launch_x(const PassXArgs& a, int ny, cudaStream_t s, int* grid_out) {
+  return a.xs == 1 ? launch_x_xs<DT, N, MODE, 1>(a, ny, s, grid_out) : launch_x_xs<DT, N, MODE, 2>(a, ny, s, grid_out);
 }
 
 template <int DT, int N, int YMODE>

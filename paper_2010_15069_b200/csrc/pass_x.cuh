@@ -43,7 +43,7 @@ __device__ __forceinline__ cplx shfl_xor_c(cplx a, int m) { return mk(shfl_xor_d
 
 // Copy the three field rows of this CTA's LINES rows into shared memory ([field][line][x], working precision),
 // 16 bytes per cp.async; a NULL field is filled with zeros.  Every thread of the CTA takes part.
-template <int DT, int NX, int LINES>
+template <int DT, int NX, int LINES, int XS>
 __device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, size_t first_point, int first_line,
                                              int tid) {
   typedef typename Store<DT>::real real;
@@ -51,8 +51,8 @@ __device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, siz
   constexpr int NCH = FIELD_BYTES / 16;
   constexpr int NTHR = LINES * (NX / 8);
   const void* src[3] = {a.V, a.Om, a.De};
-  if (a.xs != 1) {  // strided lines: one cp.async per real
-    const int S = a.xs;
+  if (XS != 1) {  // strided lines: one cp.async per real
+    constexpr int S = XS;
 #pragma unroll
     for (int f = 0; f < 3; ++f) {
       real* dst = reinterpret_cast<real*>(fbuf) + f * (LINES * NX);
@@ -167,7 +167,7 @@ struct XSmem {
 
 // Persistent: CTA b handles the row groups b, b + gridDim.x, ...; while one group is being transformed the next
 // one (psi rows and field rows) is requested into L2, so that its loads find the data there.
-template <int DT, int NX, int LINES, int MODE>
+template <int DT, int NX, int LINES, int MODE, int XS>
 __global__ void __launch_bounds__(LINES * (NX / 8), (LINES * (NX / 8) <= 256) ? 2 : 1)
 pass_x_kernel(const PassXArgs a) {
   typedef Plan<NX> P;
@@ -198,7 +198,7 @@ pass_x_kernel(const PassXArgs a) {
   // transfer runs under the tail of the previous group instead of stalling the CTA at the head of this one.
   elem* stg = reinterpret_cast<elem*>(smem);
   // point index of position 0 of line L: lines are rows (xs = 1) or the even / odd points of a row (xs = 2)
-  const int S = a.xs;
+  constexpr int S = XS;  // == a.xs
   auto line_base = [&](int L) { return (size_t)(L / S) * NX * S + (size_t)(L % S); };
   auto issue_loads = [&](int grp) {
     const size_t lb = line_base(grp * LINES + line);
@@ -240,7 +240,7 @@ pass_x_kernel(const PassXArgs a) {
     if (MODE != MODE_FWD) {
       // the exchange buffer is idle during the real-space part: it holds the field rows meanwhile
       __syncthreads();
-      stage_fields<DT, NX, LINES>(smem, a, first_point, grp * LINES, tid);
+      stage_fields<DT, NX, LINES, XS>(smem, a, first_point, grp * LINES, tid);
       cp_async_wait_all();
       __syncthreads();
       real_space<DT, NX, LINES, MODE>(v, a, smem, line, t, c, lc, sm, so);
