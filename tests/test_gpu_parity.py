@@ -284,3 +284,47 @@ def test_config5_full_size_one_step(sp):
     got = sp.spgpe_get_psi_host(h)
     ref = orc.step(w.psi0, w.V, w.Omega, w.delta, p, 1, dt, imag)
     assert rel_l2(got, ref) < TOL_C64
+
+
+def test_config2_full_schedule(sp):
+    """Config 2 exactly as BASELINE.json states it: 256 x 256, 1000 real-time steps of 5e-4."""
+    w = wl.make_workload(2)
+    h = sp.from_workload(w)
+    p = orc.params_of(w)
+    cnt, dt, imag = w.schedule[0]
+    assert (cnt, imag) == (1000, 0)
+    sp.spgpe_step(h, cnt, dt, imag)
+    ref = orc.step(w.psi0, w.V, w.Omega, w.delta, p, cnt, dt, imag)
+    assert rel_l2(sp.spgpe_get_psi_host(h), ref) < TOL_C128
+    e_ref = orc.energy(ref, w.V, w.Omega, w.delta, p)
+    assert np.abs(sp.spgpe_energy(h) - e_ref).max() < TOL_E * np.abs(e_ref).max()
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("cfg,dtype", [(3, "c128"), (4, "c128"), (4, "c64")])
+def test_full_schedules_of_configs_3_and_4(sp, cfg, dtype):
+    """The configured step counts (5000 imaginary-time steps at 1024^2; 2000 real-time steps at 2048^2, complex128 and
+    complex64 storage), compared with the oracle at 10 % of the run and at its end.  Minutes of oracle time:
+    enabled with SPGPE_FULL=1; the results of the round's run are recorded in DESIGN.md."""
+    if not os.environ.get("SPGPE_FULL"):
+        pytest.skip("set SPGPE_FULL=1")
+    orc.set_threads(orc.max_threads())
+    w = wl.make_workload(cfg, dtype=dtype)
+    h = sp.from_workload(w)
+    p = orc.params_of(w)
+    cnt, dt, imag = w.schedule[0]
+    tol = TOL_C64 if dtype == "c64" else TOL_C128
+    targets = orc.norm(w.psi0, p)
+    ref, done = w.psi0, 0
+    for upto in (cnt // 10, cnt):
+        sp.spgpe_step(h, upto - done, dt, imag)
+        ref = orc.step(ref, w.V, w.Omega, w.delta, p, upto - done, dt, imag, targets=targets)
+        done = upto
+        err = rel_l2(sp.spgpe_get_psi_host(h), ref)
+        print(f"config {cfg} {dtype}: after {done} steps rel L2 = {err:.3e}")
+        assert err < tol
+    if dtype == "c128":
+        e_ref = orc.energy(ref, w.V, w.Omega, w.delta, p)
+        e_got = sp.spgpe_energy(h)
+        print(f"config {cfg} energy rel err = {np.abs(e_got - e_ref).max() / np.abs(e_ref).max():.3e}")
+        assert np.abs(e_got - e_ref).max() < TOL_E * np.abs(e_ref).max()
