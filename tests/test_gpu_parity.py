@@ -328,3 +328,45 @@ def test_full_schedules_of_configs_3_and_4(sp, cfg, dtype):
         e_got = sp.spgpe_energy(h)
         print(f"config {cfg} energy rel err = {np.abs(e_got - e_ref).max() / np.abs(e_ref).max():.3e}")
         assert np.abs(e_got - e_ref).max() < TOL_E * np.abs(e_ref).max()
+
+
+# ---- edges: maximum line length, degenerate calls ----
+@pytest.mark.parametrize("nx,ny", [(8192, 64), (64, 8192), (8192, 128)])
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_maximum_line_length(sp, nx, ny, dtype):
+    """8192 is the longest supported line (split into two 4096-point lines); non-square grids keep the oracle fast."""
+    psi, V, Om, De, p, _ = random_problem(nx, ny, seed=nx // 64 + ny)
+    if dtype == "c64":
+        psi = psi.astype(np.complex64).astype(np.complex128)
+        V, Om, De = (a.astype(np.float32).astype(np.float64) for a in (V, Om, De))
+    h = make_solver(sp, psi, V, Om, De, p, dtype=dtype)
+    sp.spgpe_step(h, 2, 1e-3, 0)
+    ref = orc.step(psi, V, Om, De, p, 2, 1e-3, 0)
+    assert rel_l2(sp.spgpe_get_psi_host(h), ref) < (TOL_C64 if dtype == "c64" else TOL_C128)
+    if dtype == "c128":
+        e_ref = orc.energy(ref, V, Om, De, p)
+        assert np.abs(sp.spgpe_energy(h) - e_ref).max() < TOL_E * np.abs(e_ref).max()
+
+
+def test_degenerate_calls(sp):
+    """step(0) and dt = 0 leave the state alone (dt = 0: to rounding of the unnormalised transforms); sizes above
+    8192 or not a power of two are refused; NaN in the state propagates instead of trapping."""
+    psi, V, Om, De, p, _ = random_problem(128, 64, seed=8)
+    h = make_solver(sp, psi, V, Om, De, p)
+    sp.spgpe_step(h, 0, 1e-3, 0)
+    assert rel_l2(sp.spgpe_get_psi_host(h), psi) == 0.0
+    sp.spgpe_step(h, 3, 0.0, 0)
+    assert rel_l2(sp.spgpe_get_psi_host(h), psi) < 1e-14
+    for bad in ((16384, 64), (64, 96), (32, 64)):
+        with pytest.raises(sp.SpgpeError) as e:
+            sp.spgpe_create(bad[0], bad[1], 1.0, 1.0)
+        assert e.value.code == -2
+    with pytest.raises(sp.SpgpeError) as e:
+        sp.spgpe_step(h, -1, 1e-3, 0)
+    assert e.value.code == -1
+    bad_psi = psi.copy()
+    bad_psi[3, 5, 0] = np.nan
+    h2 = make_solver(sp, bad_psi, V, Om, De, p)
+    sp.spgpe_step(h2, 1, 1e-3, 0)
+    out = sp.spgpe_get_psi_host(h2)
+    assert np.isnan(out[:, :, 0].real).all()  # one NaN reaches every point of its component through the 2-D transform
