@@ -152,6 +152,12 @@ __device__ __forceinline__ void copy_table_async(double2* dst, const double2* sr
   for (int i = tid; i < n; i += nthreads) cp_async16(dst + i, src + i);
 }
 
+// ask L2 to fetch the box of the tensor map at (c0, c1): spreads the DRAM reads of the next tile over the time the
+// current one is being transformed (the later tma_load_2d then finds the data in L2)
+__device__ __forceinline__ void tma_prefetch_2d(const void* tmap, int c0, int c1) {
+  asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(tmap), "r"(c0), "r"(c1) : "memory");
+}
+
 // ---- dynamic work distribution of the persistent pass kernels -------------------------------------------------
 // sched[0] = number of groups handed out beyond the first gridDim.x, sched[1] = CTAs that have finished.  CTA b
 // starts with group b and then takes gridDim.x + atomicAdd(sched[0], 1), so that fast SMs take more groups than

@@ -111,7 +111,13 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
     const size_t e0 = ((size_t)t * nx + col) * 2 + c;  // element (row t, column col, component c)
     // the next group is requested now and published before the last barrier of this iteration (latency hidden)
     int nxt_req = 0;
-    if (tid == 0) nxt_req = sched_next(a.sched);
+    if (tid == 0) {
+      nxt_req = sched_next(a.sched);
+      if (nxt_req < ngroups) {
+#pragma unroll
+        for (int b = 0; b < NY / BR; ++b) tma_prefetch_2d(&a.tmap, nxt_req * LINES * 4, b * BR);
+      }
+    }
     mbar_wait(&mbar, it & 1);
     if (YMODE == YMODE_INVONLY) {
 #pragma unroll
