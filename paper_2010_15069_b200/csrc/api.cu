@@ -35,7 +35,7 @@ struct spgpe_ctx {
   int tab_imag;
   bool tab_valid;
   double *partial, *scale, *target, *dout;
-  CUtensorMap tmap_psi, tmap_scratch;  // column-pass tensor maps of psi and of the energy scratch buffer
+  CUtensorMap tmap_psi, tmap_scratch, tmap_psi_db;  // column-pass tensor maps of psi and of the energy scratch buffer
   int* sched;    // [4] work counters of the persistent kernels: row pass [0..1], column pass [2..3]
   double2 *ones, *wcx, *wcy;  // split axes: k_x table of ones for the row pass, join twiddles
   int *fpx, *fpy;             // split axes: true frequency of a sub-transform position
@@ -278,6 +278,7 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
     }
   }
   if (e == cudaSuccess) e = make_col_tmap(h, h->psi, plan_lines_y(h->my), &h->tmap_psi);
+  if (e == cudaSuccess && plan_lines_ydb(h->my) > 0) e = make_col_tmap(h, h->psi, plan_lines_ydb(h->my), &h->tmap_psi_db);
   if (e != cudaSuccess) {
     spgpe_destroy(h);
     return cuda_fail(e);
@@ -422,7 +423,7 @@ extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
   xa.fmax = h->fmax; xa.sched = h->sched;
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
-  ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx * h->sy; ya.sched = h->sched + 2; ya.tmap = h->tmap_psi;
+  ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx * h->sy; ya.sched = h->sched + 2; ya.tmap = h->tmap_psi; ya.tmap_db = h->tmap_psi_db;
   const double w = (h->Lx / h->nx) * (h->Ly / h->ny);
   if (!imag) {
     CK(dispatch_x(h, MODE_PRO, xa));

@@ -65,6 +65,7 @@ template <> struct Store<0> {
     return reinterpret_cast<const double*>(base)[idx];
   }
   static __device__ __forceinline__ cplx cv(double2 e) { return mk(e.x, e.y); }
+  static __device__ __forceinline__ double2 el(cplx c) { return make_double2(c.re, c.im); }
 };
 template <> struct Store<1> {
   typedef float real;
@@ -83,6 +84,7 @@ template <> struct Store<1> {
     return (double)reinterpret_cast<const float*>(base)[idx];
   }
   static __device__ __forceinline__ cplx cv(float2 e) { return mk((double)e.x, (double)e.y); }
+  static __device__ __forceinline__ float2 el(cplx c) { return make_float2((float)c.re, (float)c.im); }
 };
 
 // ---- asynchronous copies ------------------------------------------------------------------------------------
@@ -151,6 +153,16 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 __device__ __forceinline__ void copy_table_async(double2* dst, const double2* src, int n, int tid, int nthreads) {
   for (int i = tid; i < n; i += nthreads) cp_async16(dst + i, src + i);
 }
+
+// 2-D tile shared -> global (bulk async group); the shared-memory source may be reused after tma_store_wait_read
+__device__ __forceinline__ void tma_store_2d(const void* tmap, int c0, int c1, const void* smem_src) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];" ::"l"(tmap), "r"(c0),
+               "r"(c1), "r"(smem_u32(smem_src))
+               : "memory");
+}
+__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
 // ask L2 to fetch the box of the tensor map at (c0, c1): spreads the DRAM reads of the next tile over the time the
 // current one is being transformed (the later tma_load_2d then finds the data in L2)

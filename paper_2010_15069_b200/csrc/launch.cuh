@@ -11,6 +11,7 @@ namespace spgpe {
 template <int N> struct Lines {
   static constexpr int X = (N >= 2048) ? 1 : (N == 1024 ? 2 : 4);
   static constexpr int Y = (N >= 4096) ? 1 : (N >= 1024 ? 2 : 4);
+  static constexpr int YDB = (N == 2048) ? 1 : (N == 1024 ? 2 : 0);  // columns per tile of pass_y_db_kernel (0: none)
 };
 
 // number of CTAs that can be resident on the device at once (persistent row pass)
@@ -90,6 +91,32 @@ cudaError_t launch_y(const PassYArgs& a, cudaStream_t s, int* grid_out) {
   return launch_pdl(k, grid, L * (N / 8), smem, s, a);
 }
 
+template <int DT, int N>
+cudaError_t launch_y_db(const PassYArgs& a, cudaStream_t s, int* grid_out) {
+  constexpr int L = Lines<N>::YDB > 0 ? Lines<N>::YDB : 1;
+  auto k = pass_y_db_kernel<DT, N, L>;
+  constexpr size_t smem = YSmemDB<N, L>::BYTES;
+  static int resident = 0;
+  if (resident == 0) {
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    e = resident_ctas(k, L * (N / 8), smem, &resident);
+    if (e != cudaSuccess) return e;
+  }
+  const int groups = a.nx / L;
+  const int grid = groups < resident ? groups : resident;
+  *grid_out = grid;
+  return launch_pdl(k, grid, L * (N / 8), smem, s, a);
+}
+// YMODE_STEP goes to the double-buffered kernel where one exists
+template <int DT, int N>
+cudaError_t launch_y_step(const PassYArgs& a, cudaStream_t s, int* g) {
+  if constexpr (Lines<N>::YDB > 0) {
+    if (!getenv("SPGPE_DEBUG_NO_YDB")) return launch_y_db<DT, N>(a, s, g);
+  }
+  return launch_y<DT, N, YMODE_STEP>(a, s, g);
+}
+
 #define SPGPE_DEFINE_LAUNCHERS(N_)                                                               \
   cudaError_t launch_pass_x_##N_(int dt, int mode, const PassXArgs& a, int ny, cudaStream_t s, int* g) { \
     if (dt == 0) {                                                                               \
@@ -110,14 +137,14 @@ cudaError_t launch_y(const PassYArgs& a, cudaStream_t s, int* grid_out) {
   cudaError_t launch_pass_y_##N_(int dt, int ymode, const PassYArgs& a, cudaStream_t s, int* g) { \
     if (dt == 0) {                                                                               \
       switch (ymode) {                                                                           \
-        case YMODE_STEP: return launch_y<0, N_, YMODE_STEP>(a, s, g);                            \
+        case YMODE_STEP: return launch_y_step<0, N_>(a, s, g);                            \
         case YMODE_ENERGY: return launch_y<0, N_, YMODE_ENERGY>(a, s, g);                        \
         case YMODE_FWDONLY: return launch_y<0, N_, YMODE_FWDONLY>(a, s, g);                      \
         default: return launch_y<0, N_, YMODE_INVONLY>(a, s, g);                                 \
       }                                                                                          \
     }                                                                                            \
     switch (ymode) {                                                                             \
-      case YMODE_STEP: return launch_y<1, N_, YMODE_STEP>(a, s, g);                              \
+      case YMODE_STEP: return launch_y_step<1, N_>(a, s, g);                              \
       case YMODE_ENERGY: return launch_y<1, N_, YMODE_ENERGY>(a, s, g);                          \
       case YMODE_FWDONLY: return launch_y<1, N_, YMODE_FWDONLY>(a, s, g);                        \
       default: return launch_y<1, N_, YMODE_INVONLY>(a, s, g);                                   \

@@ -30,6 +30,7 @@ struct PassYArgs {
   int* sched;           // [2] device: work counter (common.cuh, sched_next)
   // psi as a 2-D tensor [NY rows][4 nx reals], box = [min(NY, 256) rows][4 LINES reals]: the columns of a group
   CUtensorMap tmap;
+  CUtensorMap tmap_db;  // the same tensor with the box of the double-buffered kernel (pass_y_db_kernel)
 };
 
 template <int NY, int LINES>
@@ -197,6 +198,118 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
       for (int i = 0; i < nw; ++i) s0 += red[i];
       a.partial[blockIdx.x] = s0;
     }
+  }
+}
+
+// ---- double-buffered variant of YMODE_STEP ------------------------------------------------------------------------
+// One 256-thread CTA per SM works on tiles of LINES columns with a staging buffer next to the line buffers: the TMA
+// load of the next tile is issued as soon as the current one has been taken out of the staging buffer, a whole tile
+// period ahead, and the results leave through the (then idle) line buffers with a TMA store.  No warp ever issues a
+// global load or store, and the DRAM traffic is spread over the whole period instead of coming in bursts between
+// the transforms.
+template <int NY, int LINES>
+struct YSmemDB {
+  static constexpr int EBUF = LINES * YLayout<NY, LINES>::LINE_PTS * 2;  // double2 elements
+  static constexpr int STG = NY * LINES * 2;                             // staging, in double2 elements (c128)
+  static constexpr int TW = tw_total<NY>();
+  static constexpr size_t BYTES = (size_t)(EBUF + STG + TW + NY) * 16;
+  static constexpr bool FITS = BYTES <= 227u * 1024u;
+};
+
+// CTA-wide exchanges; before the first one of a tile the line buffers must have been released by the TMA store of
+// the previous tile (thread 0 waits for it, the barrier tells the others)
+struct StoreDrainSync {
+  mutable bool pending;
+  int tid;
+  __device__ __forceinline__ void sync() const { __syncthreads(); }
+  __device__ __forceinline__ void acquire() const {
+    if (pending) {
+      if (tid == 0) tma_store_wait_read();
+      __syncthreads();
+      pending = false;
+    }
+  }
+  __device__ __forceinline__ void release() const {}
+};
+
+template <int DT, int NY, int LINES>
+__global__ void __launch_bounds__(LINES * (NY / 8), 1) pass_y_db_kernel(const __grid_constant__ PassYArgs a) {
+  typedef Plan<NY> P;
+  typedef Store<DT> St;
+  typedef typename St::elem elem;
+  typedef YSmemDB<NY, LINES> SM;
+  extern __shared__ __align__(128) double2 smem[];
+  constexpr int T = P::T;
+  constexpr int NTHR = LINES * (NY / 8);
+  constexpr int BR = NY < 256 ? NY : 256;
+  constexpr unsigned TILE_BYTES = (unsigned)NY * LINES * 2 * (unsigned)sizeof(elem);
+  const int tid = threadIdx.x;
+  const int c = tid & 1;
+  const int line = (tid >> 1) % LINES;
+  const int t = (tid >> 1) / LINES;
+  double2* buf = smem + (size_t)line * (YLayout<NY, LINES>::LINE_PTS * 2);
+  elem* out = reinterpret_cast<elem*>(smem);             // results leave through the line buffers
+  elem* stg = reinterpret_cast<elem*>(smem + SM::EBUF);  // the next tile arrives here
+  double2* twS = smem + SM::EBUF + SM::STG;
+  double2* eyS = twS + SM::TW;
+  __shared__ __align__(8) unsigned long long mbar;
+  __shared__ int next_s[2];
+  pdl_launch_dependents();
+  copy_table_async(twS, a.tw, SM::TW, tid, NTHR);
+  copy_table_async(eyS, a.eyk, NY, tid, NTHR);
+  const int ngroups = a.nx / LINES;
+  auto issue_loads = [&](int grp) {  // thread 0 only
+    fence_proxy_async();
+    mbar_expect_tx(&mbar, TILE_BYTES);
+#pragma unroll
+    for (int b = 0; b < NY / BR; ++b)
+      tma_load_2d(stg + (size_t)b * BR * LINES * 2, &a.tmap_db, grp * LINES * 4, b * BR, &mbar);
+  };
+  if (tid == 0) {
+    mbar_init(&mbar, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  pdl_wait();
+  if (tid == 0 && (int)blockIdx.x < ngroups) issue_loads(blockIdx.x);
+  cp_async_wait_all();
+  __syncthreads();
+  cplx v[16];
+  int it = 0;
+  for (int grp = blockIdx.x; grp < ngroups; ++it) {
+    if (tid == 0) next_s[it & 1] = sched_next(a.sched);
+    mbar_wait(&mbar, it & 1);
+#pragma unroll
+    for (int n = 0; n < 16; ++n) v[n] = St::cv(stg[((t + n * T) * LINES + line) * 2 + c]);
+    __syncthreads();  // the staging buffer is free; next_s is visible
+    const int nxt_grp = next_s[it & 1];
+    if (tid == 0 && nxt_grp < ngroups) issue_loads(nxt_grp);
+
+    const StoreDrainSync sy = {it > 0, tid};  // the first exchange waits for the previous tile's store to drain
+    line_fft_fwd<NY>(buf, twS, t, c, v, 0, sy);
+#pragma unroll
+    for (int g = 0; g < P::G; ++g)
+#pragma unroll
+      for (int s = 0; s < P::RL; ++s) {
+        const double2 f = eyS[(t + g * T) + (NY / P::RL) * s];
+        v[g * P::RL + s] = cmul(v[g * P::RL + s], mk(f.x, f.y));
+      }
+    auto hook = [&]() { __syncthreads(); };  // every warp has done its last read of the line buffers
+    line_fft_inv<NY>(buf, twS, t, c, v, 0, hook);
+#pragma unroll
+    for (int n = 0; n < 16; ++n) out[((t + n * T) * LINES + line) * 2 + c] = St::el(v[n]);
+    fence_proxy_async();  // these generic-proxy writes are read by the TMA store
+    __syncthreads();
+    if (tid == 0) {
+#pragma unroll
+      for (int b = 0; b < NY / BR; ++b)
+        tma_store_2d(&a.tmap_db, grp * LINES * 4, b * BR, out + (size_t)b * BR * LINES * 2);
+      tma_store_commit();
+    }
+    grp = nxt_grp;
+  }
+  if (tid == 0) {
+    tma_store_wait_all();
+    sched_finish(a.sched);
   }
 }
 

@@ -25,6 +25,7 @@ PlanInfo plan_info(int n) {
 
 
 int plan_lines_y(int n) { return plan_info(n).lines_y; }
+int plan_lines_ydb(int n) { return n == 2048 ? Lines<2048>::YDB : (n == 1024 ? Lines<1024>::YDB : 0); }
 
 int plan_tw_total(int n) {
   PlanInfo p = plan_info(n);
