@@ -212,7 +212,7 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
   h->hc.cb_d = 0.5 * (p->g_ud - p->g_dd);
   h->prof_ev = new std::vector<cudaEvent_t>();
   h->prof_cls = new std::vector<int>();
-  h->partial_cap = 4 * (nx > ny ? nx : ny);
+  h->partial_cap = 4 * (nx > ny ? nx : ny);  // >= 2 doubles per row group of the row pass (at most 2 ny groups)
   if (h->partial_cap < 4 * 2048) h->partial_cap = 4 * 2048;
 
   cudaError_t e = cudaSuccess;
@@ -438,7 +438,7 @@ extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
       CK(kspace_part(h, ya));
       CK(dispatch_x(h, MODE_EPI, xa));
       h->launches++;
-      CK(aux_norm_scale(h->partial, h->xgrid, w, h->target, h->p.norm_mode, h->scale, h->stream));
+      CK(aux_norm_scale(h->partial, h->ny * h->sx / plan_lines_x(h->mx), w, h->target, h->p.norm_mode, h->scale, h->stream));
     }
     h->launches++;
     CK(aux_apply_scale(h->dt, h->psi, h->points, h->scale, h->stream));

@@ -27,7 +27,7 @@ struct PassXArgs {
   const double2* tw;     // twiddles of NX
   const double2* exk;    // [2][NX] k_x phase in stored order (MODE_PRO, MODE_MID)
   const double* scale;   // [2] per-component factor applied at load (MODE_PRO, imaginary time) or NULL
-  double* partial;       // [gridDim.x][2] sum |psi_c|^2 over this CTA's rows (MODE_EPI with want_norm)
+  double* partial;       // [ny / LINES][2] sum |psi_c|^2 of every row group (MODE_EPI with want_norm)
   double tau;            // half-step size dt/2
   HalfCoef hc;
   int imag;
@@ -218,6 +218,7 @@ pass_x_kernel(const PassXArgs a) {
   };
   if ((int)blockIdx.x < ngroups) issue_loads(blockIdx.x);
 
+  __shared__ double red[2][32];
   __shared__ int next_s[2];  // group this CTA takes next (written by thread 0, double-buffered over iterations)
   int it = 0;
   for (int grp = blockIdx.x; grp < ngroups; ++it) {
@@ -245,7 +246,27 @@ pass_x_kernel(const PassXArgs a) {
       __syncthreads();
       real_space<DT, NX, LINES, MODE>(v, a, smem, line, t, c, lc, sm, so);
       if (MODE == MODE_EPI && tid == 0) next_s[it & 1] = nxt_req;
+      if (MODE == MODE_EPI && a.want_norm) {
+        // norm partials of this row group, one slot per group: the sums do not depend on which CTA took the group,
+        // so the reduction order (and every imaginary-time result) is the same from run to run.  Each lane summed
+        // its own and the other component over its 8 points: sort into (up, down) first.
+        double su = c ? so : sm, sd = c ? sm : so;
+        sm = 0.0;
+        so = 0.0;
+#pragma unroll
+        for (int m = 16; m >= 1; m >>= 1) {
+          su += shfl_xor_d(su, m);
+          sd += shfl_xor_d(sd, m);
+        }
+        if ((tid & 31) == 0) { red[0][tid >> 5] = su; red[1][tid >> 5] = sd; }
+      }
       __syncthreads();
+      if (MODE == MODE_EPI && a.want_norm && tid == 0) {
+        double s0 = 0.0, s1 = 0.0;
+        for (int i = 0; i < NTHR / 32; ++i) { s0 += red[0][i]; s1 += red[1][i]; }
+        a.partial[2 * grp] = s0;
+        a.partial[2 * grp + 1] = s1;
+      }
     }
 
     int nxt_grp;
@@ -286,25 +307,6 @@ pass_x_kernel(const PassXArgs a) {
   }
   if (tid == 0) sched_finish(a.sched);
 
-  if (MODE == MODE_EPI && a.want_norm) {
-    // each lane summed its own and the other component over its 8 points of every row: sort into (up, down)
-    double su = c ? so : sm, sd = c ? sm : so;
-    __shared__ double red[2][32];
-#pragma unroll
-    for (int m = 16; m >= 1; m >>= 1) {
-      su += shfl_xor_d(su, m);
-      sd += shfl_xor_d(sd, m);
-    }
-    const int w = tid >> 5, nw = (blockDim.x + 31) >> 5;
-    if ((tid & 31) == 0) { red[0][w] = su; red[1][w] = sd; }
-    __syncthreads();
-    if (tid == 0) {
-      double s0 = 0.0, s1 = 0.0;
-      for (int i = 0; i < nw; ++i) { s0 += red[0][i]; s1 += red[1][i]; }
-      a.partial[2 * blockIdx.x] = s0;
-      a.partial[2 * blockIdx.x + 1] = s1;
-    }
-  }
 }
 
 }  // namespace spgpe

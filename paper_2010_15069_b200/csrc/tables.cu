@@ -25,6 +25,17 @@ PlanInfo plan_info(int n) {
 
 
 int plan_lines_y(int n) { return plan_info(n).lines_y; }
+int plan_lines_x(int n) {
+  switch (n) {
+    case 64: return Lines<64>::X;
+    case 128: return Lines<128>::X;
+    case 256: return Lines<256>::X;
+    case 512: return Lines<512>::X;
+    case 1024: return Lines<1024>::X;
+    case 2048: return Lines<2048>::X;
+    default: return Lines<4096>::X;
+  }
+}
 int plan_lines_ydb(int n) { return n == 2048 ? Lines<2048>::YDB : (n == 1024 ? Lines<1024>::YDB : 0); }
 
 int plan_tw_total(int n) {

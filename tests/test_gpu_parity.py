@@ -370,3 +370,17 @@ def test_degenerate_calls(sp):
     sp.spgpe_step(h2, 1, 1e-3, 0)
     out = sp.spgpe_get_psi_host(h2)
     assert np.isnan(out[:, :, 0].real).all()  # one NaN reaches every point of its component through the 2-D transform
+
+
+def test_runs_are_bit_reproducible(sp):
+    """Rows and tiles are handed out dynamically, but every reduction has a fixed order: two runs of the same
+    imaginary-time and real-time schedule give bit-identical states and norms."""
+    w = wl.make_workload(3, n=512)
+    outs = []
+    for _ in range(2):
+        h = sp.from_workload(w)
+        sp.spgpe_step(h, 20, 1e-3, 1)
+        sp.spgpe_step(h, 20, 1e-3, 0)
+        outs.append((sp.spgpe_get_psi_host(h).copy(), sp.spgpe_norm(h), sp.spgpe_energy(h)))
+    assert np.array_equal(outs[0][0], outs[1][0])
+    assert np.array_equal(outs[0][1], outs[1][1]) and np.array_equal(outs[0][2], outs[1][2])
