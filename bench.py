@@ -296,6 +296,8 @@ def run_ours(args, wname):
         bytes_pt = [2 * 2 * esz + nfields * rsz, 2 * 2 * esz]  # row pass: psi r+w + fields; column pass: psi r+w
         achieved = bytes_pt[dom] * P / (avg[dom] * 1e-3) / 1e9
         step_bytes = (bytes_pt[0] + bytes_pt[1]) * P
+        flops_pt = 20.0 * np.log2(float(P)) + 360.0
+        dfma_tf = sp.spgpe_probe_dfma(stream.cuda_stream)
         line = {
             "metric": METRIC, "value": world * P * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
             "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -314,6 +316,12 @@ def run_ours(args, wname):
                          "algorithmic_bytes": bytes_pt[dom] * P, "peak_source": peak_src,
                          "avg_launch_us": {"row_pass": 1e3 * avg[0], "column_pass": 1e3 * avg[1]},
                          "launches_timed": kcnt, "bytes_per_point": bytes_pt},
+            # second bound of BASELINE.json's roofline definition: nominal flops (20 log2(P) + 360 per point and step,
+            # SURVEY.md 8(d)) against the FP64 FMA peak measured on this device by spgpe_probe_dfma
+            "roofline_fp64": {"bound": "alu", "achieved": flops_pt * P / (ms / K * 1e-3) / 1e12, "peak": dfma_tf,
+                              "unit": "TFLOP/s", "frac": flops_pt * P / (ms / K * 1e-3) / 1e12 / dfma_tf,
+                              "flops_per_point_step": flops_pt,
+                              "peak_source": "measured in this run (DFMA loop, 2 flops per FMA)"},
             "e2e": {"value": world * P * K / e2e_s, "unit": UNIT,
                     "h2d_bytes_per_step": (psi_bytes + nfields * P * rsz) / K, "d2h_bytes_per_step": psi_bytes / K,
                     "job": f"fields + psi host->device, spgpe_step({K}), psi device->host; {e2e_s:.4f} s"},
