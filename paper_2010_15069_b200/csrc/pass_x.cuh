@@ -51,7 +51,7 @@ __device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, siz
   constexpr int NCH = FIELD_BYTES / 16;
   constexpr int NTHR = LINES * (NX / 8);
   const void* src[3] = {a.V, a.Om, a.De};
-  if (XS != 1) {  // strided lines: one cp.async per real
+  if constexpr (XS != 1) {  // strided lines: one cp.async per real
     constexpr int S = XS;
 #pragma unroll
     for (int f = 0; f < 3; ++f) {
@@ -63,18 +63,19 @@ __device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, siz
         else dst[k] = (real)0;
       }
     }
-    return;
-  }
+  } else {
 #pragma unroll
-  for (int f = 0; f < 3; ++f) {
-    char* dst = reinterpret_cast<char*>(fbuf) + f * FIELD_BYTES;
-    if (src[f] != nullptr) {
-      const char* g = reinterpret_cast<const char*>(src[f]) + first_point * sizeof(real);
+    for (int f = 0; f < 3; ++f) {
+      char* dst = reinterpret_cast<char*>(fbuf) + f * FIELD_BYTES;
+      if (src[f] != nullptr) {
+        const char* g = reinterpret_cast<const char*>(src[f]) + first_point * sizeof(real);
 #pragma unroll
-      for (int k = tid; k < NCH; k += NTHR) cp_async16(dst + k * 16, g + k * 16);
-    } else {
+        for (int k = tid; k < NCH; k += NTHR) cp_async16(dst + k * 16, g + k * 16);
+      } else {
 #pragma unroll
-      for (int k = tid; k < NCH; k += NTHR) *reinterpret_cast<float4*>(dst + k * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int k = tid; k < NCH; k += NTHR)
+          *reinterpret_cast<float4*>(dst + k * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
+      }
     }
   }
 }
