@@ -96,37 +96,42 @@ __device__ __forceinline__ void real_space_tier(cplx* v, const PassXArgs& a, con
   const real* fO = fV + LINES * NX;
   const real* fD = fO + LINES * NX;
   const double tau = a.tau, tau2 = a.tau * a.tau;
+  // the other component of the lane's 8 points arrives first (one batch of shuffles), then the points are
+  // evaluated without touching the shuffle / shared-memory path, then the other component goes back in one batch
+  cplx o[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) o[i] = shfl_xor_c(v[8 + i], 1);
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     cplx m = v[i];
-    cplx o = shfl_xor_c(v[8 + i], 1);
     const double Vv = St::lds(fV, i * T);
     const double hO = 0.5 * St::lds(fO, i * T);
     const double hD = lc.hs * St::lds(fD, i * T);
     if (MODE == MODE_MID) {
-      const double a1 = su2_apply<false, TIER>(m, o, Vv, hO, hD, tau, tau2, lc);
-      const double a2 = su2_apply<false, TIER>(m, o, Vv, hO, hD, tau, tau2, lc);
+      const double a1 = su2_apply<false, TIER>(m, o[i], Vv, hO, hD, tau, tau2, lc);
+      const double a2 = su2_apply<false, TIER>(m, o[i], Vv, hO, hD, tau, tau2, lc);
       double pr, pi;
       phase_eval<TIER>((a1 + a2) * tau, pr, pi);
-      apply_phase(m, o, pr, pi);
+      apply_phase(m, o[i], pr, pi);
     } else if (a.imag) {
-      const double a1 = su2_apply<true, TIER>(m, o, Vv, hO, hD, tau, tau2, lc);
+      const double a1 = su2_apply<true, TIER>(m, o[i], Vv, hO, hD, tau, tau2, lc);
       const double e = exp(-a1 * tau);
       m = mk(m.re * e, m.im * e);
-      o = mk(o.re * e, o.im * e);
+      o[i] = mk(o[i].re * e, o[i].im * e);
     } else {
-      const double a1 = su2_apply<false, TIER>(m, o, Vv, hO, hD, tau, tau2, lc);
+      const double a1 = su2_apply<false, TIER>(m, o[i], Vv, hO, hD, tau, tau2, lc);
       double pr, pi;
       phase_eval<TIER>(a1 * tau, pr, pi);
-      apply_phase(m, o, pr, pi);
+      apply_phase(m, o[i], pr, pi);
     }
     if (MODE == MODE_EPI) {
       sm += fma(m.re, m.re, m.im * m.im);
-      so += fma(o.re, o.re, o.im * o.im);
+      so += fma(o[i].re, o[i].re, o[i].im * o[i].im);
     }
     v[i] = m;
-    v[8 + i] = shfl_xor_c(o, 1);
   }
+#pragma unroll
+  for (int i = 0; i < 8; ++i) v[8 + i] = shfl_xor_c(o[i], 1);
 }
 
 // Tier of the warp for this row, from bounds that hold for every point the warp touches:
