@@ -421,10 +421,10 @@ extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
   xa.tw = h->tw_x; xa.exk = h->sx == 1 ? h->exk : h->ones; xa.scale = nullptr; xa.partial = h->partial;
   xa.tau = 0.5 * dt; xa.hc = h->hc; xa.imag = imag; xa.want_norm = imag; xa.ny = h->ny * h->sx; xa.xs = h->sx;
   xa.fmax = h->fmax; xa.sched = h->sched;
+  xa.target = h->target; xa.scale_out = h->scale; xa.cell = (h->Lx / h->nx) * (h->Ly / h->ny); xa.norm_mode = h->p.norm_mode;
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
   ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx * h->sy; ya.sched = h->sched + 2; ya.tmap = h->tmap_psi; ya.tmap_db = h->tmap_psi_db;
-  const double w = (h->Lx / h->nx) * (h->Ly / h->ny);
   if (!imag) {
     CK(dispatch_x(h, MODE_PRO, xa));
     for (int s = 1; s <= n; ++s) {
@@ -436,9 +436,7 @@ extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
       xa.scale = (s > 0) ? h->scale : nullptr;  // rescale of the previous step, applied at load
       CK(dispatch_x(h, MODE_PRO, xa));
       CK(kspace_part(h, ya));
-      CK(dispatch_x(h, MODE_EPI, xa));
-      h->launches++;
-      CK(aux_norm_scale(h->partial, h->ny * h->sx / plan_lines_x(h->mx), w, h->target, h->p.norm_mode, h->scale, h->stream));
+      CK(dispatch_x(h, MODE_EPI, xa));  // also writes the rescale factors (last CTA)
     }
     h->launches++;
     CK(aux_apply_scale(h->dt, h->psi, h->points, h->scale, h->stream));

@@ -72,33 +72,6 @@ cudaError_t aux_sum_partials(const double* partial, int nblk, int ncol, double f
   return cudaGetLastError();
 }
 
-// imaginary-time renormalisation factors (R-7)
-__global__ void norm_scale_kernel(const double* __restrict__ partial, int nblk, double w,
-                                  const double* __restrict__ target, int norm_mode, double* scale) {
-  __shared__ double red[2][32];
-  double x[2] = {0.0, 0.0};
-  for (int b = threadIdx.x; b < nblk; b += blockDim.x) {
-    x[0] += partial[2 * (size_t)b];
-    x[1] += partial[2 * (size_t)b + 1];
-  }
-  double r[2];
-  block_reduce<2>(x, r, red);
-  if (threadIdx.x == 0) {
-    const double nu = w * r[0], nd = w * r[1];
-    if (norm_mode == 0) {
-      scale[0] = sqrt(target[0] / nu);
-      scale[1] = sqrt(target[1] / nd);
-    } else {
-      scale[0] = scale[1] = sqrt((target[0] + target[1]) / (nu + nd));
-    }
-  }
-}
-cudaError_t aux_norm_scale(const double* partial, int nblk, double w, const double* target, int norm_mode,
-                           double* scale, cudaStream_t s) {
-  norm_scale_kernel<<<1, 256, 0, s>>>(partial, nblk, w, target, norm_mode, scale);
-  return cudaGetLastError();
-}
-
 template <int DT>
 __global__ void apply_scale_kernel(void* psi, size_t points, const double* __restrict__ scale) {
   const double s0 = scale[0], s1 = scale[1];

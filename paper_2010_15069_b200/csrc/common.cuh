@@ -175,13 +175,16 @@ __device__ __forceinline__ void tma_prefetch_2d(const void* tmap, int c0, int c1
 // starts with group b and then takes gridDim.x + atomicAdd(sched[0], 1), so that fast SMs take more groups than
 // slow ones.  The last CTA to finish resets both words for the next launch (launches on one stream are serial).
 __device__ __forceinline__ int sched_next(int* sched) { return (int)gridDim.x + atomicAdd(&sched[0], 1); }
-__device__ __forceinline__ void sched_finish(int* sched) {
+// returns true in the CTA that finishes last (every other CTA's global writes are visible to it)
+__device__ __forceinline__ bool sched_finish(int* sched) {
   __threadfence();
   if (atomicAdd(&sched[1], 1) == (int)gridDim.x - 1) {
     sched[0] = 0;
     sched[1] = 0;
     __threadfence();
+    return true;
   }
+  return false;
 }
 
 // ---- transform plan: N = 16 * 16 * ... * R_LAST, every thread holds 16 points of one component ----

@@ -50,9 +50,6 @@ cudaError_t aux_phase_tables(const double* Kx, const double* Ky, int nx, int ny,
 // partial[nblk][ncol] -> out[col] = factor * sum_blk partial[blk][col]   (fixed summation order)
 cudaError_t aux_sum_partials(const double* partial, int nblk, int ncol, double factor, double* out,
                              cudaStream_t s);
-// scale[c] = sqrt(target[c] / (w * sum_blk partial[blk][c]))  (per component) or common factor (total)
-cudaError_t aux_norm_scale(const double* partial, int nblk, double w, const double* target, int norm_mode,
-                           double* scale, cudaStream_t s);
 cudaError_t aux_apply_scale(int dt, void* psi, size_t points, const double* scale, cudaStream_t s);
 // partial[nblk][2]: sum |psi_c|^2 ; returns nblk used through *nblk (<= max_blk)
 cudaError_t aux_norm_partials(int dt, const void* psi, size_t points, double* partial, int nblk,

@@ -35,6 +35,10 @@ struct PassXArgs {
   int ny;                // number of lines (rows x xs)
   int xs;                // 1: a line is a row; 2: a line is every second point of a row (split transform, api.cu)
   int* sched;            // [2] device: work counter (common.cuh, sched_next)
+  const double* target;  // [2] device: norm targets (MODE_EPI with want_norm)
+  double* scale_out;     // [2] device: rescale factors written by the last CTA (MODE_EPI with want_norm)
+  double cell;           // dx dy
+  int norm_mode;         // SPGPE_NORM_PER_COMPONENT | SPGPE_NORM_TOTAL
   const double* fmax;    // [3] device: max |V|, max |Omega|, max |delta| over the grid (tier bounds)
 };
 
@@ -311,7 +315,43 @@ pass_x_kernel(const PassXArgs a) {
     }
     grp = nxt_grp;
   }
-  if (tid == 0) sched_finish(a.sched);
+  if (MODE == MODE_EPI) {
+    // imaginary time (a6): the CTA that finishes last turns the per-group norm partials into the rescale factors
+    // of the next step (fixed summation order), so no separate kernel is needed
+    __shared__ int last_s;
+    if (tid == 0) last_s = sched_finish(a.sched) ? 1 : 0;
+    if (a.want_norm) {
+      __syncthreads();
+      if (last_s) {
+        double x0 = 0.0, x1 = 0.0;
+        for (int b = tid; b < ngroups; b += NTHR) {
+          x0 += __ldcg(a.partial + 2 * (size_t)b);
+          x1 += __ldcg(a.partial + 2 * (size_t)b + 1);
+        }
+#pragma unroll
+        for (int m = 16; m >= 1; m >>= 1) {
+          x0 += shfl_xor_d(x0, m);
+          x1 += shfl_xor_d(x1, m);
+        }
+        if ((tid & 31) == 0) { red[0][tid >> 5] = x0; red[1][tid >> 5] = x1; }
+        __syncthreads();
+        if (tid == 0) {
+          double nu = 0.0, nd = 0.0;
+          for (int i = 0; i < NTHR / 32; ++i) { nu += red[0][i]; nd += red[1][i]; }
+          nu *= a.cell;
+          nd *= a.cell;
+          if (a.norm_mode == 0) {
+            a.scale_out[0] = sqrt(a.target[0] / nu);
+            a.scale_out[1] = sqrt(a.target[1] / nd);
+          } else {
+            a.scale_out[0] = a.scale_out[1] = sqrt((a.target[0] + a.target[1]) / (nu + nd));
+          }
+        }
+      }
+    }
+  } else {
+    if (tid == 0) sched_finish(a.sched);
+  }
 
 }
 
