@@ -108,10 +108,12 @@ cudaError_t launch_y_db(const PassYArgs& a, cudaStream_t s, int* grid_out) {
   *grid_out = grid;
   return launch_pdl(k, grid, L * (N / 8), smem, s, a);
 }
-// YMODE_STEP goes to the double-buffered kernel where one exists
+// YMODE_STEP goes to the double-buffered kernel where one exists.  complex64 storage keeps the two-column kernel:
+// a one-column tile of float2 pairs is only 16 bytes wide, too narrow for efficient TMA boxes (measured at 2048^2:
+// 86 us against 78 us).
 template <int DT, int N>
 cudaError_t launch_y_step(const PassYArgs& a, cudaStream_t s, int* g) {
-  if constexpr (Lines<N>::YDB > 0) {
+  if constexpr (Lines<N>::YDB > 0 && DT == 0) {
     if (!getenv("SPGPE_DEBUG_NO_YDB")) return launch_y_db<DT, N>(a, s, g);
   }
   return launch_y<DT, N, YMODE_STEP>(a, s, g);
