@@ -150,7 +150,10 @@ __device__ __forceinline__ void twiddle(const double2* tw, int t, cplx* v, int f
 // acquire()/release(): bracket every exchange (the shared-memory stores, the barrier and the loads after it).
 // CtaSync: the whole CTA works on the same lines, no bracket.  GroupSync (pass_x.cuh): two thread groups of one
 // CTA work on different lines and take turns at their exchanges.
+// REG_TW1: the policy object carries the thread's 15 stage-1 twiddles in registers (tw1[k-1] = w_1[k][lo]); used by
+// kernels with registers to spare, it takes those reads off the shared-memory path.
 struct CtaSync {
+  static constexpr bool REG_TW1 = false;
   __device__ __forceinline__ void sync() const { __syncthreads(); }
   __device__ __forceinline__ void acquire() const {}
   __device__ __forceinline__ void release() const {}
@@ -161,13 +164,32 @@ __device__ __forceinline__ void sync_last_p(const Sy& sy) {
   else sy.sync();
 }
 
+// stage-1 twiddles from registers (see REG_TW1)
+template <int D>
+__device__ __forceinline__ void twiddle_reg(const double2* w, cplx* v, int flip) {
+#pragma unroll
+  for (int k = 1; k < 16; ++k) {
+    double2 d = w[k - 1];
+    if (k & 1) {
+      d.x = flip_sign(d.x, flip);
+      d.y = flip_sign(d.y, flip);
+    }
+    v[k] = (D < 0) ? cmul(v[k], mk(d.x, d.y)) : cmulc(v[k], mk(d.x, d.y));
+  }
+}
+template <int N, int J, int D, typename Sy>
+__device__ __forceinline__ void twiddle_p(const double2* tw, int t, cplx* v, int flip, const Sy& sy) {
+  if constexpr (Sy::REG_TW1 && J == 1) twiddle_reg<D>(sy.tw1, v, flip);
+  else twiddle<N, J, D>(tw, t, v, flip);
+}
+
 // one forward radix-16 stage J followed by the exchange into stage J+1's (or the last stage's) registers
 template <int N, int J, typename Sy>
 __device__ __forceinline__ void fwd_stages(double2* buf, const double2* tw, int t, int c, cplx* v, int flip,
                                            const Sy& sy) {
   if constexpr (J < Plan<N>::NS) {
     dft16<-1>(v);
-    twiddle<N, J, -1>(tw, t, v, flip);
+    twiddle_p<N, J, -1>(tw, t, v, flip, sy);
     sy.acquire();
     sts_stage<N, J>(buf, t, c, v);
     if constexpr (J + 1 < Plan<N>::NS) {
@@ -208,7 +230,7 @@ __device__ __forceinline__ void inv_stages(double2* buf, const double2* tw, int 
     lds_stage<N, J>(buf, t, c, v);
     sy.release();
     if constexpr (J == 1) hook();
-    twiddle<N, J, +1>(tw, t, v, flip);
+    twiddle_p<N, J, +1>(tw, t, v, flip, sy);
     dft16<+1>(v);
     inv_stages<N, J - 1>(buf, tw, t, c, v, flip, hook, sy);
   }

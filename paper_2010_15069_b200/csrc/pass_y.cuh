@@ -219,8 +219,10 @@ struct YSmemDB {
 // CTA-wide exchanges; before the first one of a tile the line buffers must have been released by the TMA store of
 // the previous tile (thread 0 waits for it, the barrier tells the others)
 struct StoreDrainSync {
+  static constexpr bool REG_TW1 = true;
   mutable bool pending;
   int tid;
+  double2 tw1[15];  // the thread's stage-1 twiddles (this kernel has registers to spare: 256 threads per SM)
   __device__ __forceinline__ void sync() const { __syncthreads(); }
   __device__ __forceinline__ void acquire() const {
     if (pending) {
@@ -273,6 +275,18 @@ __global__ void __launch_bounds__(LINES * (NY / 8), 1) pass_y_db_kernel(const __
   if (tid == 0 && (int)blockIdx.x < ngroups) issue_loads(blockIdx.x);
   cp_async_wait_all();
   __syncthreads();
+  // per-thread constants kept in registers for the whole kernel: the k_y phases of the thread's 16 stored positions
+  // and its 15 stage-1 twiddles
+  StoreDrainSync sy;
+  sy.tid = tid;
+  sy.pending = false;
+#pragma unroll
+  for (int k = 1; k < 16; ++k) sy.tw1[k - 1] = twS[tw_offset<NY>(1) + (k - 1) * (NY >> 4) + t];
+  double2 eyr[16];
+#pragma unroll
+  for (int g = 0; g < P::G; ++g)
+#pragma unroll
+    for (int s = 0; s < P::RL; ++s) eyr[g * P::RL + s] = eyS[(t + g * T) + (NY / P::RL) * s];
   cplx v[16];
   int it = 0;
   for (int grp = blockIdx.x; grp < ngroups; ++it) {
@@ -284,17 +298,17 @@ __global__ void __launch_bounds__(LINES * (NY / 8), 1) pass_y_db_kernel(const __
     const int nxt_grp = next_s[it & 1];
     if (tid == 0 && nxt_grp < ngroups) issue_loads(nxt_grp);
 
-    const StoreDrainSync sy = {it > 0, tid};  // the first exchange waits for the previous tile's store to drain
+    sy.pending = it > 0;  // the first exchange waits for the previous tile's store to drain
     line_fft_fwd<NY>(buf, twS, t, c, v, 0, sy);
 #pragma unroll
     for (int g = 0; g < P::G; ++g)
 #pragma unroll
       for (int s = 0; s < P::RL; ++s) {
-        const double2 f = eyS[(t + g * T) + (NY / P::RL) * s];
+        const double2 f = eyr[g * P::RL + s];
         v[g * P::RL + s] = cmul(v[g * P::RL + s], mk(f.x, f.y));
       }
     auto hook = [&]() { __syncthreads(); };  // every warp has done its last read of the line buffers
-    line_fft_inv<NY>(buf, twS, t, c, v, 0, hook);
+    line_fft_inv<NY>(buf, twS, t, c, v, 0, hook, sy);
 #pragma unroll
     for (int n = 0; n < 16; ++n) out[((t + n * T) * LINES + line) * 2 + c] = St::el(v[n]);
     fence_proxy_async();  // these generic-proxy writes are read by the TMA store
