@@ -90,7 +90,7 @@ __device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, siz
 // component at its own point), evaluates the half-step(s) in the (mine, other) basis (su2.cuh, LaneCoef) and
 // sends the other component back.  Fields come from shared memory (stage_fields), index lx = line*NX + x.
 // TIER: evaluation tier of su2.cuh, guaranteed by the caller for every point of the warp.
-template <int DT, int NX, int LINES, int MODE, int TIER>
+template <int DT, int NX, int LINES, int MODE, int TIER, bool BZ0>
 __device__ __forceinline__ void real_space_tier(cplx* v, const PassXArgs& a, const void* fbuf, int line, int t, int c,
                                                 const LaneCoef& lc, double& sm, double& so) {
   typedef Store<DT> St;
@@ -112,18 +112,18 @@ __device__ __forceinline__ void real_space_tier(cplx* v, const PassXArgs& a, con
     const double hO = 0.5 * St::lds(fO, i * T);
     const double hD = lc.hs * St::lds(fD, i * T);
     if (MODE == MODE_MID) {
-      const double a1 = su2_apply<false, TIER>(m, o[i], Vv, hO, hD, tau, tau2, lc);
-      const double a2 = su2_apply<false, TIER>(m, o[i], Vv, hO, hD, tau, tau2, lc);
+      const double a1 = su2_apply<false, TIER, BZ0>(m, o[i], Vv, hO, hD, tau, tau2, lc);
+      const double a2 = su2_apply<false, TIER, BZ0>(m, o[i], Vv, hO, hD, tau, tau2, lc);
       double pr, pi;
       phase_eval<TIER>((a1 + a2) * tau, pr, pi);
       apply_phase(m, o[i], pr, pi);
     } else if (a.imag) {
-      const double a1 = su2_apply<true, TIER>(m, o[i], Vv, hO, hD, tau, tau2, lc);
+      const double a1 = su2_apply<true, TIER, BZ0>(m, o[i], Vv, hO, hD, tau, tau2, lc);
       const double e = exp(-a1 * tau);
       m = mk(m.re * e, m.im * e);
       o[i] = mk(o[i].re * e, o[i].im * e);
     } else {
-      const double a1 = su2_apply<false, TIER>(m, o[i], Vv, hO, hD, tau, tau2, lc);
+      const double a1 = su2_apply<false, TIER, BZ0>(m, o[i], Vv, hO, hD, tau, tau2, lc);
       double pr, pi;
       phase_eval<TIER>(a1 * tau, pr, pi);
       apply_phase(m, o[i], pr, pi);
@@ -152,20 +152,30 @@ __device__ __forceinline__ int row_tier(const cplx* v, const PassXArgs& a, const
   const double z = (a.tau * a.tau) * fma(bx, bx, bz * bz);
   const double x = (MODE == MODE_MID ? 2.0 : 1.0) * a.tau * fma(fmax(fabs(lc.cam), fabs(lc.cao)), NT, a.fmax[0]);
   const bool ph_ok = (x * x <= SPGPE_Z_FAST);
-  const bool t0 = ph_ok && (z <= SPGPE_Z_TINY);  // NaN fails every test and lands in the general tier
-  const bool t1 = ph_ok && (z <= SPGPE_Z_FAST);
+  const bool t0 = ph_ok && (z <= SPGPE_Z_MICRO);  // NaN fails every test and lands in the general tier
+  const bool t1 = ph_ok && (z <= SPGPE_Z_TINY);
+  const bool t2 = ph_ok && (z <= SPGPE_Z_FAST);
   if (__all_sync(0xffffffffu, t0)) return 0;
   if (__all_sync(0xffffffffu, t1)) return 1;
-  return 2;
+  if (__all_sync(0xffffffffu, t2)) return 2;
+  return 3;
 }
 
 template <int DT, int NX, int LINES, int MODE>
 __device__ __forceinline__ void real_space(cplx* v, const PassXArgs& a, const void* fbuf, int line, int t, int c,
                                            const LaneCoef& lc, double& sm, double& so) {
   const int tier = row_tier<MODE>(v, a, lc);
-  if (tier == 0) real_space_tier<DT, NX, LINES, MODE, 0>(v, a, fbuf, line, t, c, lc, sm, so);
-  else if (tier == 1) real_space_tier<DT, NX, LINES, MODE, 1>(v, a, fbuf, line, t, c, lc, sm, so);
-  else real_space_tier<DT, NX, LINES, MODE, 2>(v, a, fbuf, line, t, c, lc, sm, so);
+  if (a.hc.cb_u == 0.0 && a.hc.cb_d == 0.0) {  // all g equal: b_z has no density term
+    if (tier == 0) real_space_tier<DT, NX, LINES, MODE, 0, true>(v, a, fbuf, line, t, c, lc, sm, so);
+    else if (tier == 1) real_space_tier<DT, NX, LINES, MODE, 1, true>(v, a, fbuf, line, t, c, lc, sm, so);
+    else if (tier == 2) real_space_tier<DT, NX, LINES, MODE, 2, true>(v, a, fbuf, line, t, c, lc, sm, so);
+    else real_space_tier<DT, NX, LINES, MODE, 3, true>(v, a, fbuf, line, t, c, lc, sm, so);
+  } else {
+    if (tier == 0) real_space_tier<DT, NX, LINES, MODE, 0, false>(v, a, fbuf, line, t, c, lc, sm, so);
+    else if (tier == 1) real_space_tier<DT, NX, LINES, MODE, 1, false>(v, a, fbuf, line, t, c, lc, sm, so);
+    else if (tier == 2) real_space_tier<DT, NX, LINES, MODE, 2, false>(v, a, fbuf, line, t, c, lc, sm, so);
+    else real_space_tier<DT, NX, LINES, MODE, 3, false>(v, a, fbuf, line, t, c, lc, sm, so);
+  }
 }
 
 // dynamic shared memory of the row pass: LINES padded line buffers, then the twiddle table

@@ -8,6 +8,7 @@
 // z = +theta^2.  Writing sin(theta)/|b| = tau S(z) needs no square root, no division and no |b| -> 0 special case.
 //
 // Evaluation tiers:
+//   |z| <= 2^-20 : series to degree 2 (first dropped term z^3/6! < 1.3e-21)
 //   |z| <= 2^-13 : series to degree 3 (first dropped term z^4/8! < 6e-21)
 //   |z| <= 1/4   : series to degree 7 (first dropped term z^8/16! < 8e-19)
 //   otherwise    : libm sincos / cosh / sinh
@@ -22,8 +23,17 @@ struct HalfCoef {
   double ca_u, ca_d, cb_u, cb_d;  // (g_uu+g_ud)/2, (g_dd+g_ud)/2, (g_uu-g_ud)/2, (g_ud-g_dd)/2
 };
 
+#define SPGPE_Z_MICRO 9.5367431640625e-07
 #define SPGPE_Z_TINY 0.0001220703125
 #define SPGPE_Z_FAST 0.25
+
+// C(z), S(z) to degree 2
+__device__ __forceinline__ void cs_series2(double z, double& C, double& S) {
+  const double c = fma(z, 1.0 / 24.0, 0.5);
+  const double s = fma(z, 1.0 / 120.0, 1.0 / 6.0);
+  C = fma(c, z, 1.0);
+  S = fma(s, z, 1.0);
+}
 
 // C(z), S(z) to degree 3
 __device__ __forceinline__ void cs_series3(double z, double& C, double& S) {
@@ -72,12 +82,14 @@ __device__ __noinline__ double2 cs_general(double z) {
   return make_double2(C, S);
 }
 
-// TIER 0: |z| <= SPGPE_Z_TINY guaranteed by the caller; 1: |z| <= SPGPE_Z_FAST guaranteed; 2: anything
+// TIER 0: |z| <= SPGPE_Z_MICRO guaranteed by the caller; 1: |z| <= SPGPE_Z_TINY; 2: |z| <= SPGPE_Z_FAST; 3: anything
 template <bool IMAG, int TIER>
 __device__ __forceinline__ void cs_eval(double z, double& C, double& S) {
   if (TIER == 0) {
-    cs_series3(z, C, S);
+    cs_series2(z, C, S);
   } else if (TIER == 1) {
+    cs_series3(z, C, S);
+  } else if (TIER == 2) {
     cs_series7(z, C, S);
   } else {
     const double2 r = cs_general<IMAG>(z);
@@ -86,7 +98,7 @@ __device__ __forceinline__ void cs_eval(double z, double& C, double& S) {
   }
 }
 
-// e^{-i x} = (cos x, -sin x); TIER 0/1: x^2 <= SPGPE_Z_FAST guaranteed by the caller (series to degree 7)
+// e^{-i x} = (cos x, -sin x); TIER 0-2: x^2 <= SPGPE_Z_FAST guaranteed by the caller (series to degree 7)
 static __device__ __noinline__ double2 phase_general(double x) {
   double sn, cn;
   sincos(x, &sn, &cn);
@@ -94,7 +106,7 @@ static __device__ __noinline__ double2 phase_general(double x) {
 }
 template <int TIER>
 __device__ __forceinline__ void phase_eval(double x, double& pr, double& pi) {
-  if (TIER == 2) {
+  if (TIER == 3) {
     const double2 r = phase_general(x);
     pr = r.x;
     pi = r.y;
@@ -128,13 +140,14 @@ __device__ __forceinline__ LaneCoef lane_coef(const HalfCoef& hc, int c) {
 
 // Apply the traceless part M = C 1 - (i) tau S (b.sigma) to (m, o) with the densities of (m, o); returns a (the
 // scalar part of H_loc) so that the caller applies e^{-i a tau} / e^{-a tau}.
-template <bool IMAG, int TIER>
+// BZ0: g_uu = g_dd = g_ud, so b_z carries no density term (cbm = cbo = 0).
+template <bool IMAG, int TIER, bool BZ0>
 __device__ __forceinline__ double su2_apply(cplx& m, cplx& o, double V, double hO, double hDs, double tau,
                                             double tau2, const LaneCoef& lc) {
   const double nm = fma(m.re, m.re, m.im * m.im);
   const double no = fma(o.re, o.re, o.im * o.im);
   const double a = fma(lc.cam, nm, fma(lc.cao, no, V));
-  const double bz = fma(lc.cbm, nm, fma(lc.cbo, no, hDs));
+  const double bz = BZ0 ? hDs : fma(lc.cbm, nm, fma(lc.cbo, no, hDs));
   const double th2 = tau2 * fma(hO, hO, bz * bz);
   double C, S;
   cs_eval<IMAG, TIER>(IMAG ? th2 : -th2, C, S);
