@@ -111,7 +111,14 @@ __device__ __forceinline__ void real_space_tier(cplx* v, const PassXArgs& a, con
     const double Vv = St::lds(fV, i * T);
     const double hO = 0.5 * St::lds(fO, i * T);
     const double hD = lc.hs * St::lds(fD, i * T);
-    if (MODE == MODE_MID) {
+    if (MODE == MODE_MID && BZ0) {
+      // all g equal: the traceless part of H_loc holds no density and its scalar part only n_up + n_dn, which the
+      // unitary half-step conserves, so R(tau) R(tau) = R(2 tau) exactly (one evaluation; differs from two by rounding)
+      const double a1 = su2_apply<false, TIER, BZ0>(m, o[i], Vv, hO, hD, 2.0 * tau, 4.0 * tau2, lc);
+      double pr, pi;
+      phase_eval<TIER>(a1 * (2.0 * tau), pr, pi);
+      apply_phase(m, o[i], pr, pi);
+    } else if (MODE == MODE_MID) {
       const double a1 = su2_apply<false, TIER, BZ0>(m, o[i], Vv, hO, hD, tau, tau2, lc);
       const double a2 = su2_apply<false, TIER, BZ0>(m, o[i], Vv, hO, hD, tau, tau2, lc);
       double pr, pi;
@@ -141,15 +148,16 @@ __device__ __forceinline__ void real_space_tier(cplx* v, const PassXArgs& a, con
 // Tier of the warp for this row, from bounds that hold for every point the warp touches:
 //   n_up + n_dn <= NT = max_n |own v[n]|^2 + the partner's maximum (conserved by the real-time half-step),
 //   |b_z| <= max|delta|/2 + max(|cbm|, |cbo|) NT,  |b_x| <= max|Omega|/2,  |a| <= max|V| + max(|cam|, |cao|) NT.
+// merged: the two half-steps of MODE_MID are evaluated as one step of 2 tau (real_space_tier, BZ0)
 template <int MODE>
-__device__ __forceinline__ int row_tier(const cplx* v, const PassXArgs& a, const LaneCoef& lc) {
+__device__ __forceinline__ int row_tier(const cplx* v, const PassXArgs& a, const LaneCoef& lc, bool merged) {
   double nmax = 0.0;
 #pragma unroll
   for (int n = 0; n < 16; ++n) nmax = fmax(nmax, fma(v[n].re, v[n].re, v[n].im * v[n].im));
   const double NT = nmax + shfl_xor_d(nmax, 1);
   const double bz = fma(fmax(fabs(lc.cbm), fabs(lc.cbo)), NT, 0.5 * a.fmax[2]);
   const double bx = 0.5 * a.fmax[1];
-  const double z = (a.tau * a.tau) * fma(bx, bx, bz * bz);
+  const double z = (merged ? 4.0 : 1.0) * (a.tau * a.tau) * fma(bx, bx, bz * bz);
   const double x = (MODE == MODE_MID ? 2.0 : 1.0) * a.tau * fma(fmax(fabs(lc.cam), fabs(lc.cao)), NT, a.fmax[0]);
   const bool ph_ok = (x * x <= SPGPE_Z_FAST);
   const bool t0 = ph_ok && (z <= SPGPE_Z_MICRO);  // NaN fails every test and lands in the general tier
@@ -164,8 +172,9 @@ __device__ __forceinline__ int row_tier(const cplx* v, const PassXArgs& a, const
 template <int DT, int NX, int LINES, int MODE>
 __device__ __forceinline__ void real_space(cplx* v, const PassXArgs& a, const void* fbuf, int line, int t, int c,
                                            const LaneCoef& lc, double& sm, double& so) {
-  const int tier = row_tier<MODE>(v, a, lc);
-  if (a.hc.cb_u == 0.0 && a.hc.cb_d == 0.0) {  // all g equal: b_z has no density term
+  const bool bz0 = a.hc.cb_u == 0.0 && a.hc.cb_d == 0.0;
+  const int tier = row_tier<MODE>(v, a, lc, bz0 && MODE == MODE_MID);
+  if (bz0) {  // all g equal: b_z has no density term
     if (tier == 0) real_space_tier<DT, NX, LINES, MODE, 0, true>(v, a, fbuf, line, t, c, lc, sm, so);
     else if (tier == 1) real_space_tier<DT, NX, LINES, MODE, 1, true>(v, a, fbuf, line, t, c, lc, sm, so);
     else if (tier == 2) real_space_tier<DT, NX, LINES, MODE, 2, true>(v, a, fbuf, line, t, c, lc, sm, so);
