@@ -1,6 +1,7 @@
-"""Parity of the CUDA path (through the C ABI of include/spgpe.h) with the CPU oracle, element by element,
-on the same seeded inputs.  Tolerances are BASELINE.json's: relative L2 of psi <= 1e-10 (complex128),
-<= 1e-4 (complex64 storage); energy within 1e-9 relative (complex128).
+"""Parity of the CUDA path (through the C ABI of include/spgpe.h) with the CPU oracle on the same seeded inputs.
+Tolerances are BASELINE.json's: relative L2 of psi <= 1e-10 (complex128), <= 1e-4 (complex64 storage); energy within
+1e-9 relative (complex128).  Beside every L2 bound stands an element-wise one (assert_parity): max |got - ref| <=
+1e-9 max |ref| (complex128), 1e-3 max |ref| (complex64 storage).
 """
 import os
 
@@ -28,6 +29,23 @@ def sp():
 
 def rel_l2(a, b):
     return np.linalg.norm((a.astype(np.complex128) - b).ravel()) / np.linalg.norm(b.ravel())
+
+
+# element-wise bound beside the L2 one: a norm alone lets a single wrong element through at large sizes (one wrong
+# element of 8192^2 x 2 contributes 8.6e-5 to the relative L2).  max |got - ref| <= TOL_EL * max |ref|.
+TOL_EL = {TOL_C128: 1e-9, TOL_C64: 1e-3}
+
+
+def max_el(a, b):
+    return np.abs(a.astype(np.complex128) - b).max() / np.abs(b).max()
+
+
+def assert_parity(got, ref, tol):
+    """BASELINE.json's relative L2 bound and, element by element, max |got - ref| / max |ref|."""
+    assert got.shape == ref.shape
+    e2, em = rel_l2(got, ref), max_el(got, ref)
+    assert e2 < tol, f"relative L2 {e2:.3e} >= {tol:g}"
+    assert em < TOL_EL[tol], f"max element error {em:.3e} >= {TOL_EL[tol]:g} (relative L2 {e2:.3e})"
 
 
 def random_problem(nx, ny, seed, g=(1.0, 0.8, 0.6), k_L=0.7):
@@ -70,11 +88,11 @@ def test_real_time_steps_match_oracle(sp, nx, ny):
     sp.spgpe_step(h, n, dt, 0)
     got = sp.spgpe_get_psi_host(h)
     ref = orc.step(psi, V, Om, De, p, n, dt, 0)
-    assert rel_l2(got, ref) < TOL_C128
+    assert_parity(got, ref, TOL_C128)
     # step(n) then step(m) equals step(n+m)
     sp.spgpe_step(h, 2, dt, 0)
     ref2 = orc.step(ref, V, Om, De, p, 2, dt, 0)
-    assert rel_l2(sp.spgpe_get_psi_host(h), ref2) < TOL_C128
+    assert_parity(sp.spgpe_get_psi_host(h), ref2, TOL_C128)
 
 
 @pytest.mark.parametrize("nx,ny", [(64, 64), (256, 128), (128, 512), (1024, 64)])
@@ -87,7 +105,7 @@ def test_imaginary_time_steps_match_oracle(sp, nx, ny, mode):
     sp.spgpe_step(h, n, dt, 1)
     got = sp.spgpe_get_psi_host(h)
     ref = orc.step(psi, V, Om, De, p, n, dt, 1)
-    assert rel_l2(got, ref) < TOL_C128
+    assert_parity(got, ref, TOL_C128)
     np.testing.assert_allclose(sp.spgpe_norm(h), orc.norm(ref, p), rtol=1e-12)
 
 
@@ -110,7 +128,7 @@ def test_null_fields_and_zero_coupling(sp):
     h = make_solver(sp, psi, None, None, None, p)
     sp.spgpe_step(h, 5, 1e-3, 0)
     ref = orc.step(psi, None, None, None, p, 5, 1e-3, 0)
-    assert rel_l2(sp.spgpe_get_psi_host(h), ref) < TOL_C128
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C128)
 
 
 def test_negative_dt_and_large_arguments(sp):
@@ -121,11 +139,11 @@ def test_negative_dt_and_large_arguments(sp):
     h = make_solver(sp, psi, V, Om, De, p)
     sp.spgpe_step(h, 2, -5e-3, 0)
     ref = orc.step(psi, V, Om, De, p, 2, -5e-3, 0)
-    assert rel_l2(sp.spgpe_get_psi_host(h), ref) < TOL_C128
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C128)
     h2 = make_solver(sp, psi, V * 0.05, Om * 0.3, De, p)
     sp.spgpe_step(h2, 2, 5e-3, 1)
     ref2 = orc.step(psi, V * 0.05, Om * 0.3, De, p, 2, 5e-3, 1)
-    assert rel_l2(sp.spgpe_get_psi_host(h2), ref2) < TOL_C128
+    assert_parity(sp.spgpe_get_psi_host(h2), ref2, TOL_C128)
 
 
 def test_device_tensor_interface_and_stream(sp):
@@ -148,7 +166,7 @@ def test_device_tensor_interface_and_stream(sp):
         sp.spgpe_get_psi(h, out)
         sp.spgpe_synchronize(h)
     ref = orc.step(psi, V, Om, De, p, 4, 1e-3, 0)
-    assert rel_l2(out.cpu().numpy(), ref) < TOL_C128
+    assert_parity(out.cpu().numpy(), ref, TOL_C128)
 
 
 def test_error_codes(sp):
@@ -173,7 +191,7 @@ def test_c64_storage_matches_oracle(sp, nx, ny):
     h = make_solver(sp, psi, V, Om, De, p, dtype="c64")
     sp.spgpe_step(h, 20, 1e-3, 0)
     ref = orc.step(psi, V, Om, De, p, 20, 1e-3, 0)
-    assert rel_l2(sp.spgpe_get_psi_host(h), ref) < TOL_C64
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C64)
 
 
 # ---- the five workloads of BASELINE.json (proxy sizes the oracle finishes in seconds; full sizes below) ----
@@ -189,7 +207,7 @@ def test_workload_configs_proxy(sp, cfg, n, steps):
         sp.spgpe_step(h, cnt, dt, imag)
         ref = orc.step(ref, w.V, w.Omega, w.delta, p, cnt, dt, imag)
     got = sp.spgpe_get_psi_host(h)
-    assert rel_l2(got, ref) < (TOL_C64 if dtype == "c64" else TOL_C128)
+    assert_parity(got, ref, (TOL_C64 if dtype == "c64" else TOL_C128))
     if dtype == "c128":
         e_ref = orc.energy(ref, w.V, w.Omega, w.delta, p)
         e_got = sp.spgpe_energy(h)
@@ -209,7 +227,7 @@ def test_full_size_configs_few_steps(sp, cfg, dtype, steps):
     sp.spgpe_step(h, steps, dt, imag)
     got = sp.spgpe_get_psi_host(h)
     ref = orc.step(w.psi0, w.V, w.Omega, w.delta, p, steps, dt, imag)
-    assert rel_l2(got, ref) < (TOL_C64 if dtype == "c64" else TOL_C128)
+    assert_parity(got, ref, (TOL_C64 if dtype == "c64" else TOL_C128))
     np.testing.assert_allclose(sp.spgpe_norm(h), orc.norm(ref, p), rtol=1e-6 if dtype == "c64" else 1e-12)
     if dtype == "c128":
         e_ref = orc.energy(ref, w.V, w.Omega, w.delta, p)
@@ -243,7 +261,7 @@ def test_general_tier_rows_match_oracle(sp):
     h = make_solver(sp, psi, V, Om, De, p)
     sp.spgpe_step(h, 3, 4e-3, 0)
     ref = orc.step(psi, V, Om, De, p, 3, 4e-3, 0)
-    assert rel_l2(sp.spgpe_get_psi_host(h), ref) < TOL_C128
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C128)
 
 
 # ---- split axes (line lengths above 4096 are transformed as two interleaved half-length lines, split.cu) ----
@@ -261,20 +279,19 @@ def test_split_axes_small_sizes(sp, monkeypatch, nx, ny, dtype):
     h = make_solver(sp, psi, V, Om, De, p, dtype=dtype)
     sp.spgpe_step(h, 3, 2e-3, 0)
     ref = orc.step(psi, V, Om, De, p, 3, 2e-3, 0)
-    assert rel_l2(sp.spgpe_get_psi_host(h), ref) < tol
+    assert_parity(sp.spgpe_get_psi_host(h), ref, tol)
     if dtype == "c128":
         e_ref = orc.energy(ref, V, Om, De, p)
         assert np.abs(sp.spgpe_energy(h) - e_ref).max() < TOL_E * np.abs(e_ref).max()
     sp.spgpe_step(h, 2, 1e-3, 1)
     ref2 = orc.step(ref, V, Om, De, p, 2, 1e-3, 1, targets=orc.norm(psi, p))
-    assert rel_l2(sp.spgpe_get_psi_host(h), ref2) < tol
+    assert_parity(sp.spgpe_get_psi_host(h), ref2, tol)
 
 
-@pytest.mark.slow
 def test_config5_full_size_one_step(sp):
-    """Config 5 (8192 x 8192, complex64 storage): one real-time step against the oracle on every element."""
-    if not os.environ.get("SPGPE_FULL"):
-        pytest.skip("set SPGPE_FULL=1 (builds 1 GiB arrays, oracle takes minutes)")
+    """Config 5 (8192 x 8192, complex64 storage) at its stated size: one real-time step against the oracle on every
+    element (relative L2 and per-element bound), norms included.  Part of the default gpu set: building the 1 GiB
+    state and one oracle step take a few minutes of host time."""
     orc.set_threads(orc.max_threads())
     w = wl.make_workload(5)
     h = sp.from_workload(w)
@@ -283,7 +300,9 @@ def test_config5_full_size_one_step(sp):
     sp.spgpe_step(h, 1, dt, imag)
     got = sp.spgpe_get_psi_host(h)
     ref = orc.step(w.psi0, w.V, w.Omega, w.delta, p, 1, dt, imag)
-    assert rel_l2(got, ref) < TOL_C64
+    print(f"config 5 (8192^2 c64), 1 step: rel L2 = {rel_l2(got, ref):.3e}, max element = {max_el(got, ref):.3e}")
+    assert_parity(got, ref, TOL_C64)
+    np.testing.assert_allclose(sp.spgpe_norm(h), orc.norm(ref, p), rtol=1e-6)
 
 
 def test_config2_full_schedule(sp):
@@ -295,7 +314,7 @@ def test_config2_full_schedule(sp):
     assert (cnt, imag) == (1000, 0)
     sp.spgpe_step(h, cnt, dt, imag)
     ref = orc.step(w.psi0, w.V, w.Omega, w.delta, p, cnt, dt, imag)
-    assert rel_l2(sp.spgpe_get_psi_host(h), ref) < TOL_C128
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C128)
     e_ref = orc.energy(ref, w.V, w.Omega, w.delta, p)
     assert np.abs(sp.spgpe_energy(h) - e_ref).max() < TOL_E * np.abs(e_ref).max()
 
@@ -320,9 +339,10 @@ def test_full_schedules_of_configs_3_and_4(sp, cfg, dtype):
         sp.spgpe_step(h, upto - done, dt, imag)
         ref = orc.step(ref, w.V, w.Omega, w.delta, p, upto - done, dt, imag, targets=targets)
         done = upto
-        err = rel_l2(sp.spgpe_get_psi_host(h), ref)
-        print(f"config {cfg} {dtype}: after {done} steps rel L2 = {err:.3e}")
-        assert err < tol
+        got = sp.spgpe_get_psi_host(h)
+        print(f"config {cfg} {dtype}: after {done} steps rel L2 = {rel_l2(got, ref):.3e}, "
+              f"max element = {max_el(got, ref):.3e}")
+        assert_parity(got, ref, tol)
     if dtype == "c128":
         e_ref = orc.energy(ref, w.V, w.Omega, w.delta, p)
         e_got = sp.spgpe_energy(h)
@@ -342,7 +362,7 @@ def test_maximum_line_length(sp, nx, ny, dtype):
     h = make_solver(sp, psi, V, Om, De, p, dtype=dtype)
     sp.spgpe_step(h, 2, 1e-3, 0)
     ref = orc.step(psi, V, Om, De, p, 2, 1e-3, 0)
-    assert rel_l2(sp.spgpe_get_psi_host(h), ref) < (TOL_C64 if dtype == "c64" else TOL_C128)
+    assert_parity(sp.spgpe_get_psi_host(h), ref, (TOL_C64 if dtype == "c64" else TOL_C128))
     if dtype == "c128":
         e_ref = orc.energy(ref, V, Om, De, p)
         assert np.abs(sp.spgpe_energy(h) - e_ref).max() < TOL_E * np.abs(e_ref).max()
