@@ -50,7 +50,8 @@ enum {
   SPGPE_ERR_UNSUPPORTED = -2, /* nx or ny not a power of two in [64, 8192] */
   SPGPE_ERR_NOT_READY = -3,   /* step/norm/energy/get before set_psi */
   SPGPE_ERR_CUDA = -4,        /* a CUDA call failed; spgpe_last_cuda_error() gives its text */
-  SPGPE_ERR_NO_DEVICE = -5    /* no CUDA device / not an sm_100 device */
+  SPGPE_ERR_NO_DEVICE = -5,   /* no CUDA device / not an sm_100 device */
+  SPGPE_ERR_NO_MEMORY = -6    /* host or device allocation failed in spgpe_create */
 };
 
 typedef struct {
@@ -61,7 +62,9 @@ typedef struct {
 } spgpe_params;
 
 /* Create a solver for an nx x ny grid on the box of full widths Lx, Ly.  cuda_stream is a cudaStream_t
- * (NULL = the default stream); all work of the handle is enqueued on it.  Fields start as zero. */
+ * (NULL = the default stream); all work of the handle is enqueued on it.  Fields start as zero.  The handle lives on
+ * the CUDA device that is current in the calling thread; later calls may come from any thread (one at a time per
+ * handle) with any device current. */
 int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double Ly, const spgpe_params* p,
                  void* cuda_stream);
 int spgpe_destroy(spgpe_handle h);
@@ -84,7 +87,8 @@ int spgpe_get_psi_host(spgpe_handle h, void* h_psi);       /* synchronises the s
 int spgpe_set_norm_targets(spgpe_handle h, double n_up, double n_dn);
 
 /* n Strang steps of size dt.  imag != 0: imaginary time with dt = d tau > 0 and a
- * renormalisation after every step.  dt may be negative in real time.  Asynchronous.
+ * renormalisation after every step.  dt may be negative in real time; NaN or infinite dt, and dt <= 0 in imaginary
+ * time, return SPGPE_ERR_INVALID_ARG.  A component whose norm is zero keeps scale 1 (it stays zero).  Asynchronous.
  * step(n) then step(m) equals step(n+m) to rounding. */
 int spgpe_step(spgpe_handle h, int n, double dt, int imag);
 

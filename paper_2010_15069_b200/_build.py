@@ -15,6 +15,8 @@ NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
     "-Xcompiler", "-fPIC",
 ]
+# extra compiler flags for diagnostic builds, e.g. SPGPE_NVCC_EXTRA="-DSPGPE_TIMELINE" (common.cuh)
+NVCC_FLAGS += os.environ.get("SPGPE_NVCC_EXTRA", "").split()
 
 
 def _nvcc() -> str:

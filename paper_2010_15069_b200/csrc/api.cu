@@ -22,6 +22,7 @@ struct spgpe_ctx {
   double Lx, Ly;
   spgpe_params p;
   cudaStream_t stream;
+  LaunchEnv env;  // device of the handle and the diagnostic switches, read once at spgpe_create
   int dt;  // storage precision
   size_t points, field_bytes, psi_bytes;
   void* psi;
@@ -37,7 +38,7 @@ struct spgpe_ctx {
   double *partial, *scale, *target, *dout;
   CUtensorMap tmap_psi, tmap_scratch, tmap_psi_db;  // column-pass tensor maps of psi and of the energy scratch buffer
   int* sched;    // [4] work counters of the persistent kernels: row pass [0..1], column pass [2..3]
-  double2 *ones, *wcx, *wcy;  // split axes: k_x table of ones for the row pass, join twiddles
+  double2 *wcx, *wcy;         // split axes: join twiddles
   int *fpx, *fpy;             // split axes: true frequency of a sub-transform position
   double* fmax;  // [3] max |V|, |Omega|, |delta| (tier bounds of the row pass)
   int partial_cap;
@@ -77,6 +78,27 @@ static cudaError_t prof_end(spgpe_ctx* h) {
 
 static thread_local char g_cuda_err[256] = "";
 
+// Every entry point that takes a handle runs with the handle's device current and restores the caller's device on
+// return (a handle created on GPU 1 keeps working when the caller has switched to GPU 0 in between).
+struct DeviceGuard {
+  int prev;
+  bool switched;
+  cudaError_t err;
+  explicit DeviceGuard(int dev) : prev(-1), switched(false), err(cudaSuccess) {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != dev) {
+      err = cudaSetDevice(dev);
+      switched = (err == cudaSuccess);
+    }
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+};
+#define ON_DEVICE(h)                                   \
+  DeviceGuard guard__((h)->env.device);                \
+  if (guard__.err != cudaSuccess) return cuda_fail(guard__.err)
+
 static int cuda_fail(cudaError_t e) {
   snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
   return SPGPE_ERR_CUDA;
@@ -90,15 +112,16 @@ static int cuda_fail(cudaError_t e) {
 // Tensor map of a psi-shaped buffer for the column pass (pass_y.cuh): 2-D [ny rows][4 nx reals], box of
 // min(ny, 256) rows x 4 * lines reals.  The driver entry point is looked up at run time (no libcuda link).
 static cudaError_t make_col_tmap(const spgpe_ctx* h, void* base, int lines, CUtensorMap* out) {
-  static PFN_cuTensorMapEncodeTiled_v12000 encode = nullptr;
-  if (!encode) {
+  // looked up once per process (the driver entry point is the same for every device); C++11 makes the
+  // initialisation of a function-local static thread-safe
+  static const PFN_cuTensorMapEncodeTiled_v12000 encode = []() -> PFN_cuTensorMapEncodeTiled_v12000 {
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult q;
-    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q);
-    if (e != cudaSuccess) return e;
-    if (!fn || q != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
-    encode = (PFN_cuTensorMapEncodeTiled_v12000)fn;
-  }
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess) return nullptr;
+    if (!fn || q != cudaDriverEntryPointSuccess) return nullptr;
+    return (PFN_cuTensorMapEncodeTiled_v12000)fn;
+  }();
+  if (!encode) return cudaErrorNotSupported;
   const size_t rsz = (h->dt == SPGPE_C128) ? 8 : 4;
   // a split y axis is seen as my rows of sy * nx points: row r of that view holds the rows sy * r + p of the grid
   const cuuint64_t gdim[2] = {(cuuint64_t)h->nx * h->sy * 4, (cuuint64_t)h->my};
@@ -114,33 +137,34 @@ static cudaError_t make_col_tmap(const spgpe_ctx* h, void* base, int lines, CUte
 static bool size_ok(int n) { return n >= 64 && n <= 8192 && (n & (n - 1)) == 0; }
 // an axis is split when it is longer than the longest line of the pass kernels (or, for tests, when
 // SPGPE_DEBUG_SPLIT_MIN asks for it)
-static int split_of(int n) {
-  int nmin = 8192;
-  if (const char* e = getenv("SPGPE_DEBUG_SPLIT_MIN")) { const int v = atoi(e); if (v >= 128) nmin = v; }
-  return n >= nmin ? 2 : 1;
+static int split_of(int n, int nmin) { return n >= nmin ? 2 : 1; }
+// the three diagnostic environment variables are read here, once per spgpe_create
+static int env_int(const char* name) {
+  const char* e = getenv(name);
+  return e ? atoi(e) : 0;
 }
 
 static cudaError_t dispatch_x_raw(spgpe_ctx* h, int mode, const PassXArgs& a) {
   const int nl = h->ny * h->sx;  // lines
   switch (h->mx) {
-    case 64: return launch_pass_x_64(h->dt, mode, a, nl, h->stream, &h->xgrid);
-    case 128: return launch_pass_x_128(h->dt, mode, a, nl, h->stream, &h->xgrid);
-    case 256: return launch_pass_x_256(h->dt, mode, a, nl, h->stream, &h->xgrid);
-    case 512: return launch_pass_x_512(h->dt, mode, a, nl, h->stream, &h->xgrid);
-    case 1024: return launch_pass_x_1024(h->dt, mode, a, nl, h->stream, &h->xgrid);
-    case 2048: return launch_pass_x_2048(h->dt, mode, a, nl, h->stream, &h->xgrid);
-    default: return launch_pass_x_4096(h->dt, mode, a, nl, h->stream, &h->xgrid);
+    case 64: return launch_pass_x_64(h->dt, mode, a, nl, h->stream, h->env, &h->xgrid);
+    case 128: return launch_pass_x_128(h->dt, mode, a, nl, h->stream, h->env, &h->xgrid);
+    case 256: return launch_pass_x_256(h->dt, mode, a, nl, h->stream, h->env, &h->xgrid);
+    case 512: return launch_pass_x_512(h->dt, mode, a, nl, h->stream, h->env, &h->xgrid);
+    case 1024: return launch_pass_x_1024(h->dt, mode, a, nl, h->stream, h->env, &h->xgrid);
+    case 2048: return launch_pass_x_2048(h->dt, mode, a, nl, h->stream, h->env, &h->xgrid);
+    default: return launch_pass_x_4096(h->dt, mode, a, nl, h->stream, h->env, &h->xgrid);
   }
 }
 static cudaError_t dispatch_y_raw(spgpe_ctx* h, int ymode, const PassYArgs& a) {
   switch (h->my) {
-    case 64: return launch_pass_y_64(h->dt, ymode, a, h->stream, &h->ygrid);
-    case 128: return launch_pass_y_128(h->dt, ymode, a, h->stream, &h->ygrid);
-    case 256: return launch_pass_y_256(h->dt, ymode, a, h->stream, &h->ygrid);
-    case 512: return launch_pass_y_512(h->dt, ymode, a, h->stream, &h->ygrid);
-    case 1024: return launch_pass_y_1024(h->dt, ymode, a, h->stream, &h->ygrid);
-    case 2048: return launch_pass_y_2048(h->dt, ymode, a, h->stream, &h->ygrid);
-    default: return launch_pass_y_4096(h->dt, ymode, a, h->stream, &h->ygrid);
+    case 64: return launch_pass_y_64(h->dt, ymode, a, h->stream, h->env, &h->ygrid);
+    case 128: return launch_pass_y_128(h->dt, ymode, a, h->stream, h->env, &h->ygrid);
+    case 256: return launch_pass_y_256(h->dt, ymode, a, h->stream, h->env, &h->ygrid);
+    case 512: return launch_pass_y_512(h->dt, ymode, a, h->stream, h->env, &h->ygrid);
+    case 1024: return launch_pass_y_1024(h->dt, ymode, a, h->stream, h->env, &h->ygrid);
+    case 2048: return launch_pass_y_2048(h->dt, ymode, a, h->stream, h->env, &h->ygrid);
+    default: return launch_pass_y_4096(h->dt, ymode, a, h->stream, h->env, &h->ygrid);
   }
 }
 
@@ -196,10 +220,15 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
   if (major != 10) return SPGPE_ERR_NO_DEVICE;
 
   spgpe_ctx* h = new (std::nothrow) spgpe_ctx();
-  if (!h) return SPGPE_ERR_INVALID_ARG;
+  if (!h) return SPGPE_ERR_NO_MEMORY;
   memset(h, 0, sizeof(*h));
   h->nx = nx; h->ny = ny; h->Lx = Lx; h->Ly = Ly; h->p = *p;
-  h->sx = split_of(nx); h->sy = split_of(ny); h->mx = nx / h->sx; h->my = ny / h->sy;
+  h->env.device = dev;
+  h->env.ctas_per_sm = env_int("SPGPE_DEBUG_CTAS_PER_SM");
+  h->env.no_ydb = env_int("SPGPE_DEBUG_NO_YDB");
+  int split_min = env_int("SPGPE_DEBUG_SPLIT_MIN");
+  if (split_min < 128) split_min = 8192;
+  h->sx = split_of(nx, split_min); h->sy = split_of(ny, split_min); h->mx = nx / h->sx; h->my = ny / h->sy;
   h->stream = (cudaStream_t)cuda_stream;
   h->dt = p->dtype;
   h->points = (size_t)nx * ny;
@@ -210,8 +239,14 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
   h->hc.ca_d = 0.5 * (p->g_dd + p->g_ud);
   h->hc.cb_u = 0.5 * (p->g_uu - p->g_ud);
   h->hc.cb_d = 0.5 * (p->g_ud - p->g_dd);
-  h->prof_ev = new std::vector<cudaEvent_t>();
-  h->prof_cls = new std::vector<int>();
+  h->prof_ev = new (std::nothrow) std::vector<cudaEvent_t>();
+  h->prof_cls = new (std::nothrow) std::vector<int>();
+  if (!h->prof_ev || !h->prof_cls) {
+    delete h->prof_ev;
+    delete h->prof_cls;
+    delete h;
+    return SPGPE_ERR_NO_MEMORY;
+  }
   h->partial_cap = 4 * (nx > ny ? nx : ny);  // >= 2 doubles per row group of the row pass (at most 2 ny groups)
   if (h->partial_cap < 4 * 2048) h->partial_cap = 4 * 2048;
 
@@ -271,17 +306,12 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
     alloc((void**)dwc, sizeof(double2) * m);
     if (e == cudaSuccess) e = cudaMemcpy(*dfp, fp.data(), sizeof(int) * m, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(*dwc, wc.data(), sizeof(double2) * m, cudaMemcpyHostToDevice);
-    if (ax == 0) {
-      std::vector<double2> one(2 * (size_t)m, make_double2(1.0, 0.0));
-      alloc((void**)&h->ones, sizeof(double2) * one.size());
-      if (e == cudaSuccess) e = cudaMemcpy(h->ones, one.data(), sizeof(double2) * one.size(), cudaMemcpyHostToDevice);
-    }
   }
   if (e == cudaSuccess) e = make_col_tmap(h, h->psi, plan_lines_y(h->my), &h->tmap_psi);
   if (e == cudaSuccess && plan_lines_ydb(h->my) > 0) e = make_col_tmap(h, h->psi, plan_lines_ydb(h->my), &h->tmap_psi_db);
   if (e != cudaSuccess) {
     spgpe_destroy(h);
-    return cuda_fail(e);
+    return e == cudaErrorMemoryAllocation ? SPGPE_ERR_NO_MEMORY : cuda_fail(e);
   }
   *out = h;
   return SPGPE_OK;
@@ -289,9 +319,10 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
 
 extern "C" int spgpe_destroy(spgpe_handle h) {
   if (!h) return SPGPE_ERR_INVALID_ARG;
+  ON_DEVICE(h);
   cudaStreamSynchronize(h->stream);
   void* ptrs[] = {h->psi, h->scratch, h->Vbuf, h->Ombuf, h->Debuf, h->tw_x, h->tw_y, h->Kx, h->Ky,
-                  h->exk, h->eyk, h->partial, h->scale, h->target, h->dout, h->fmax, h->sched, h->ones, h->wcx, h->wcy, h->fpx, h->fpy};
+                  h->exk, h->eyk, h->partial, h->scale, h->target, h->dout, h->fmax, h->sched, h->wcx, h->wcy, h->fpx, h->fpy};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   if (h->prof_ev) {
@@ -305,6 +336,7 @@ extern "C" int spgpe_destroy(spgpe_handle h) {
 
 static int set_field(spgpe_handle h, const void* src, void* buf, const void** slot, cudaMemcpyKind kind) {
   if (!h) return SPGPE_ERR_INVALID_ARG;
+  ON_DEVICE(h);
   const int which = (buf == h->Vbuf) ? 0 : (buf == h->Ombuf ? 1 : 2);
   if (!src) {
     *slot = nullptr;
@@ -347,6 +379,7 @@ static int norms_to(spgpe_handle h, double* d_out2) {
 
 static int set_psi_common(spgpe_handle h, const void* src, cudaMemcpyKind kind) {
   if (!h || !src) return SPGPE_ERR_INVALID_ARG;
+  ON_DEVICE(h);
   CK(cudaMemcpyAsync(h->psi, src, h->psi_bytes, kind, h->stream));
   if (kind == cudaMemcpyHostToDevice) CK(cudaStreamSynchronize(h->stream));
   h->ready = true;
@@ -357,12 +390,14 @@ extern "C" int spgpe_set_psi_host(spgpe_handle h, const void* p) { return set_ps
 
 extern "C" int spgpe_get_psi(spgpe_handle h, void* d) {
   if (!h || !d) return SPGPE_ERR_INVALID_ARG;
+  ON_DEVICE(h);
   if (!h->ready) return SPGPE_ERR_NOT_READY;
   CK(cudaMemcpyAsync(d, h->psi, h->psi_bytes, cudaMemcpyDeviceToDevice, h->stream));
   return SPGPE_OK;
 }
 extern "C" int spgpe_get_psi_host(spgpe_handle h, void* p) {
   if (!h || !p) return SPGPE_ERR_INVALID_ARG;
+  ON_DEVICE(h);
   if (!h->ready) return SPGPE_ERR_NOT_READY;
   CK(cudaMemcpyAsync(p, h->psi, h->psi_bytes, cudaMemcpyDeviceToHost, h->stream));
   CK(cudaStreamSynchronize(h->stream));
@@ -370,6 +405,7 @@ extern "C" int spgpe_get_psi_host(spgpe_handle h, void* p) {
 }
 extern "C" int spgpe_set_norm_targets(spgpe_handle h, double n_up, double n_dn) {
   if (!h || !(n_up > 0.0) || !(n_dn > 0.0)) return SPGPE_ERR_INVALID_ARG;
+  ON_DEVICE(h);
   h->launches++;
   CK(aux_set_targets(h->target, n_up, n_dn, h->stream));
   return SPGPE_OK;
@@ -409,22 +445,26 @@ static cudaError_t kspace_part(spgpe_ctx* h, const PassYArgs& ya) {
 }
 
 extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
-  if (!h || n < 0 || !(dt == dt)) return SPGPE_ERR_INVALID_ARG;
+  if (!h || n < 0 || !(dt == dt) || isinf(dt)) return SPGPE_ERR_INVALID_ARG;
+  imag = imag ? 1 : 0;
+  if (imag && !(dt > 0.0)) return SPGPE_ERR_INVALID_ARG;  // imaginary time: dt = d tau > 0 (spgpe.h)
   if (!h->ready) return SPGPE_ERR_NOT_READY;
   if (n == 0) return SPGPE_OK;
-  imag = imag ? 1 : 0;
+  ON_DEVICE(h);
   int rc = ensure_tables(h, dt, imag);
   if (rc) return rc;
   PassXArgs xa;
   memset(&xa, 0, sizeof(xa));
   xa.src = h->psi; xa.dst = h->psi; xa.V = h->V; xa.Om = h->Om; xa.De = h->De;
-  xa.tw = h->tw_x; xa.exk = h->sx == 1 ? h->exk : h->ones; xa.scale = nullptr; xa.partial = h->partial;
+  xa.tw = h->tw_x; xa.scale = nullptr; xa.partial = h->partial;
   xa.tau = 0.5 * dt; xa.hc = h->hc; xa.imag = imag; xa.want_norm = imag; xa.ny = h->ny * h->sx; xa.xs = h->sx;
   xa.fmax = h->fmax; xa.sched = h->sched;
   xa.target = h->target; xa.scale_out = h->scale; xa.cell = (h->Lx / h->nx) * (h->Ly / h->ny); xa.norm_mode = h->p.norm_mode;
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
-  ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx * h->sy; ya.sched = h->sched + 2; ya.tmap = h->tmap_psi; ya.tmap_db = h->tmap_psi_db;
+  ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx * h->sy;
+  // the k_x phase rides on the column pass unless a split axis sends the k-space phases to the join kernel
+  ya.exk = (h->sx == 1 && h->sy == 1) ? h->exk : nullptr; ya.sched = h->sched + 2; ya.tmap = h->tmap_psi; ya.tmap_db = h->tmap_psi_db;
   if (!imag) {
     CK(dispatch_x(h, MODE_PRO, xa));
     for (int s = 1; s <= n; ++s) {
@@ -446,6 +486,7 @@ extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
 
 extern "C" int spgpe_norm(spgpe_handle h, double out[2]) {
   if (!h || !out) return SPGPE_ERR_INVALID_ARG;
+  ON_DEVICE(h);
   if (!h->ready) return SPGPE_ERR_NOT_READY;
   int rc = norms_to(h, h->dout);
   if (rc) return rc;
@@ -456,6 +497,7 @@ extern "C" int spgpe_norm(spgpe_handle h, double out[2]) {
 
 extern "C" int spgpe_energy(spgpe_handle h, double out[5]) {
   if (!h || !out) return SPGPE_ERR_INVALID_ARG;
+  ON_DEVICE(h);
   if (!h->ready) return SPGPE_ERR_NOT_READY;
   if (!h->scratch) {
     CK(cudaMalloc(&h->scratch, h->psi_bytes));
@@ -496,11 +538,13 @@ extern "C" int spgpe_energy(spgpe_handle h, double out[5]) {
 
 extern "C" int spgpe_synchronize(spgpe_handle h) {
   if (!h) return SPGPE_ERR_INVALID_ARG;
+  ON_DEVICE(h);
   CK(cudaStreamSynchronize(h->stream));
   return SPGPE_OK;
 }
 extern "C" int spgpe_profile(spgpe_handle h, int enable) {
   if (!h) return SPGPE_ERR_INVALID_ARG;
+  ON_DEVICE(h);
   CK(cudaStreamSynchronize(h->stream));
   h->prof_on = enable != 0;
   h->prof_used = 0;
@@ -508,6 +552,7 @@ extern "C" int spgpe_profile(spgpe_handle h, int enable) {
 }
 extern "C" int spgpe_profile_read(spgpe_handle h, double ms[2], long long count[2]) {
   if (!h || !ms || !count) return SPGPE_ERR_INVALID_ARG;
+  ON_DEVICE(h);
   CK(cudaStreamSynchronize(h->stream));
   ms[0] = ms[1] = 0.0;
   count[0] = count[1] = 0;
@@ -531,6 +576,7 @@ extern "C" const char* spgpe_strerror(int code) {
     case SPGPE_ERR_NOT_READY: return "no order parameter set (call spgpe_set_psi first)";
     case SPGPE_ERR_CUDA: return "CUDA error (see spgpe_last_cuda_error)";
     case SPGPE_ERR_NO_DEVICE: return "no sm_100 CUDA device";
+    case SPGPE_ERR_NO_MEMORY: return "out of host or device memory";
     default: return "unknown error code";
   }
 }

@@ -4,7 +4,37 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+// Phase timeline of the pass kernels (diagnostic builds only: nvcc -DSPGPE_TIMELINE).  Thread 0 of CTA 0 sums the
+// cycles between successive marks over all its tiles and prints them once per launch.  Compiled out by default.
+#ifdef SPGPE_TIMELINE
+#include <stdio.h>
+#define TL_DECL(n) long long tl_[n] = {}; long long tl_last_ = clock64(); int tl_n_ = 0
+#define TL_MARK(i) do { const long long now_ = clock64(); tl_[i] += now_ - tl_last_; tl_last_ = now_; } while (0)
+#define TL_TILE() (++tl_n_)
+#define TL_DUMP(name, n)                                                                     \
+  do {                                                                                       \
+    if (blockIdx.x == 0 && threadIdx.x == 0 && tl_n_ > 0) {                                  \
+      printf("TL %s tiles %d:", name, tl_n_);                                                \
+      for (int i_ = 0; i_ < n; ++i_) printf(" %lld", tl_[i_] / tl_n_);                       \
+      printf("\n");                                                                          \
+    }                                                                                        \
+  } while (0)
+#else
+#define TL_DECL(n)
+#define TL_MARK(i)
+#define TL_TILE()
+#define TL_DUMP(name, n)
+#endif
+
 namespace spgpe {
+
+// What a launcher needs to know about its handle: the device the handle lives on (the current device of the
+// calling thread during every entry point, api.cu) and the diagnostic switches read once at spgpe_create.
+struct LaunchEnv {
+  int device;        // CUDA device ordinal of the handle
+  int ctas_per_sm;   // SPGPE_DEBUG_CTAS_PER_SM: cap on resident CTAs per SM of the persistent kernels (0: none)
+  int no_ydb;        // SPGPE_DEBUG_NO_YDB: column pass without the double-buffered kernel
+};
 
 struct cplx {
   double re, im;

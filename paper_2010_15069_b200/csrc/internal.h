@@ -9,8 +9,10 @@ namespace spgpe {
 
 // per-length launchers (inst_<N>.cu)
 #define SPGPE_DECL(N_)                                                                          \
-  cudaError_t launch_pass_x_##N_(int dt, int mode, const PassXArgs& a, int ny, cudaStream_t s, int* grid); \
-  cudaError_t launch_pass_y_##N_(int dt, int ymode, const PassYArgs& a, cudaStream_t s, int* grid);
+  cudaError_t launch_pass_x_##N_(int dt, int mode, const PassXArgs& a, int ny, cudaStream_t s,           \
+                                 const LaunchEnv& env, int* grid);                                        \
+  cudaError_t launch_pass_y_##N_(int dt, int ymode, const PassYArgs& a, cudaStream_t s, const LaunchEnv& env, \
+                                 int* grid);
 SPGPE_DECL(64)
 SPGPE_DECL(128)
 SPGPE_DECL(256)
@@ -28,7 +30,7 @@ struct SplitArgs {
   const int* fy;       // [ny/2]
   const double2* wx;   // [nx/2] exp(-2 pi i fx[pos] / nx)
   const double2* wy;   // [ny/2]
-  const double2* phx;  // [2][nx] k_x phase by true frequency (split x axis only)
+  const double2* phx;  // [2][nx] k_x phase: by true frequency (split x axis) or by stored position (unsplit)
   const double2* phy;  // [ny]    k_y phase by true frequency, 1/(nx ny) included (split y axis only)
   const double* Kx;    // [2][nx] energy mode: by true frequency (split axis) or by stored position (unsplit)
   const double* Ky;    // [ny]

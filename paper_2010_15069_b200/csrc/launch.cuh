@@ -14,23 +14,38 @@ template <int N> struct Lines {
   static constexpr int YDB = (N == 2048) ? 1 : (N == 1024 ? 2 : 0);  // columns per tile of pass_y_db_kernel (0: none)
 };
 
-// number of CTAs that can be resident on the device at once (persistent row pass)
+constexpr int SPGPE_MAX_DEVICES = 64;
+
+// Number of CTAs of `kernel` that can be resident on env.device at once, and the one-time opt-in to `smem` bytes
+// of dynamic shared memory.  Both are per-device properties: the cache is indexed by the device ordinal (a second
+// handle on another GPU of the same process sets the attribute there too).  Racing threads compute the same value.
 template <typename K>
-cudaError_t resident_ctas(K kernel, int threads, size_t smem, int* out) {
-  int dev = 0, sms = 0, occ = 0;
-  cudaError_t e = cudaGetDevice(&dev);
-  if (e != cudaSuccess) return e;
-  e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  if (e != cudaSuccess) return e;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem);
-  if (e != cudaSuccess) return e;
-  if (const char* cap = getenv("SPGPE_DEBUG_CTAS_PER_SM")) { int c = atoi(cap); if (c > 0 && c < occ) occ = c; }
-  *out = sms * (occ > 0 ? occ : 1);
+cudaError_t resident_ctas(K kernel, int threads, size_t smem, const LaunchEnv& env, int* cache, int* out) {
+  const int slot = (env.device >= 0 && env.device < SPGPE_MAX_DEVICES) ? env.device : -1;
+  int r = slot >= 0 ? __atomic_load_n(&cache[slot], __ATOMIC_ACQUIRE) : 0;
+  if (r == 0) {
+    int sms = 0, occ = 0;
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, env.device);
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem);
+    if (e != cudaSuccess) return e;
+    r = sms * (occ > 0 ? occ : 1);
+    if (slot >= 0) __atomic_store_n(&cache[slot], r, __ATOMIC_RELEASE);
+  }
+  if (env.ctas_per_sm > 0) {  // diagnostic cap (not cached)
+    int sms = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, env.device);
+    if (e != cudaSuccess) return e;
+    if (env.ctas_per_sm * sms < r) r = env.ctas_per_sm * sms;
+  }
+  *out = r;
   return cudaSuccess;
 }
 
 template <int DT, int N, int MODE>
-cudaError_t launch_x(const PassXArgs& a, int ny, cudaStream_t s, int* grid_out);
+cudaError_t launch_x(const PassXArgs& a, int ny, cudaStream_t s, const LaunchEnv& env, int* grid_out);
 
 // launch with programmatic stream serialization (common.cuh, pdl_wait): the kernel may start its prologue while
 // the previous kernel on the stream drains
@@ -51,17 +66,14 @@ cudaError_t launch_pdl(K kernel, int grid, int threads, size_t smem, cudaStream_
 
 // grid_out: number of CTAs launched (= rows of PassXArgs::partial written by MODE_EPI)
 template <int DT, int N, int MODE, int XS>
-cudaError_t launch_x_xs(const PassXArgs& a, int ny, cudaStream_t s, int* grid_out) {
+cudaError_t launch_x_xs(const PassXArgs& a, int ny, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
   constexpr int L = Lines<N>::X;
   auto k = pass_x_kernel<DT, N, L, MODE, XS>;
   constexpr size_t smem = XSmem<N, L>::BYTES;
-  static int resident = 0;
-  if (resident == 0) {
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    e = resident_ctas(k, L * (N / 8), smem, &resident);
-    if (e != cudaSuccess) return e;
-  }
+  static int cache[SPGPE_MAX_DEVICES] = {};
+  int resident = 0;
+  cudaError_t e = resident_ctas(k, L * (N / 8), smem, env, cache, &resident);
+  if (e != cudaSuccess) return e;
   const int groups = ny / L;
   const int grid = groups < resident ? groups : resident;
   *grid_out = grid;
@@ -69,22 +81,20 @@ cudaError_t launch_x_xs(const PassXArgs& a, int ny, cudaStream_t s, int* grid_ou
 }
 
 template <int DT, int N, int MODE>
-cudaError_t launch_x(const PassXArgs& a, int ny, cudaStream_t s, int* grid_out) {
-  return a.xs == 1 ? launch_x_xs<DT, N, MODE, 1>(a, ny, s, grid_out) : launch_x_xs<DT, N, MODE, 2>(a, ny, s, grid_out);
+cudaError_t launch_x(const PassXArgs& a, int ny, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
+  return a.xs == 1 ? launch_x_xs<DT, N, MODE, 1>(a, ny, s, env, grid_out)
+                   : launch_x_xs<DT, N, MODE, 2>(a, ny, s, env, grid_out);
 }
 
 template <int DT, int N, int YMODE>
-cudaError_t launch_y(const PassYArgs& a, cudaStream_t s, int* grid_out) {
+cudaError_t launch_y(const PassYArgs& a, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
   constexpr int L = Lines<N>::Y;
   auto k = pass_y_kernel<DT, N, L, YMODE>;
   constexpr size_t smem = YSmem<N, L>::BYTES;
-  static int resident = 0;
-  if (resident == 0) {
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    e = resident_ctas(k, L * (N / 8), smem, &resident);
-    if (e != cudaSuccess) return e;
-  }
+  static int cache[SPGPE_MAX_DEVICES] = {};
+  int resident = 0;
+  cudaError_t e = resident_ctas(k, L * (N / 8), smem, env, cache, &resident);
+  if (e != cudaSuccess) return e;
   const int groups = a.nx / L;
   const int grid = groups < resident ? groups : resident;
   *grid_out = grid;
@@ -92,64 +102,82 @@ cudaError_t launch_y(const PassYArgs& a, cudaStream_t s, int* grid_out) {
 }
 
 template <int DT, int N>
-cudaError_t launch_y_db(const PassYArgs& a, cudaStream_t s, int* grid_out) {
+cudaError_t launch_y_db(const PassYArgs& a, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
   constexpr int L = Lines<N>::YDB > 0 ? Lines<N>::YDB : 1;
   auto k = pass_y_db_kernel<DT, N, L>;
   constexpr size_t smem = YSmemDB<N, L>::BYTES;
-  static int resident = 0;
-  if (resident == 0) {
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    e = resident_ctas(k, L * (N / 8), smem, &resident);
-    if (e != cudaSuccess) return e;
-  }
+  static int cache[SPGPE_MAX_DEVICES] = {};
+  int resident = 0;
+  cudaError_t e = resident_ctas(k, L * (N / 8), smem, env, cache, &resident);
+  if (e != cudaSuccess) return e;
   const int groups = a.nx / L;
   const int grid = groups < resident ? groups : resident;
   *grid_out = grid;
   return launch_pdl(k, grid, L * (N / 8), smem, s, a);
+}
+// experiment: one column per 256-thread CTA, two CTAs per SM (k_y phases from global memory), tensor map of the
+// double-buffered kernel (same box)
+template <int DT, int N>
+cudaError_t launch_y_2cta(PassYArgs a, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
+  auto k = pass_y_kernel<DT, N, 1, YMODE_STEP, true>;
+  constexpr size_t smem = YSmem<N, 1, true>::BYTES;
+  static int cache[SPGPE_MAX_DEVICES] = {};
+  int resident = 0;
+  cudaError_t e = resident_ctas(k, N / 8, smem, env, cache, &resident);
+  if (e != cudaSuccess) return e;
+  a.tmap = a.tmap_db;
+  const int groups = a.nx;
+  const int grid = groups < resident ? groups : resident;
+  *grid_out = grid;
+  return launch_pdl(k, grid, N / 8, smem, s, a);
 }
 // YMODE_STEP goes to the double-buffered kernel where one exists.  complex64 storage keeps the two-column kernel:
 // a one-column tile of float2 pairs is only 16 bytes wide, too narrow for efficient TMA boxes (measured at 2048^2:
 // 86 us against 78 us).
 template <int DT, int N>
-cudaError_t launch_y_step(const PassYArgs& a, cudaStream_t s, int* g) {
-  if constexpr (Lines<N>::YDB > 0 && DT == 0) {
-    if (!getenv("SPGPE_DEBUG_NO_YDB")) return launch_y_db<DT, N>(a, s, g);
+cudaError_t launch_y_step(const PassYArgs& a, cudaStream_t s, const LaunchEnv& env, int* g) {
+  if constexpr (N == 2048 && DT == 0) {
+    if (env.no_ydb == 2) return launch_y_2cta<DT, N>(a, s, env, g);
   }
-  return launch_y<DT, N, YMODE_STEP>(a, s, g);
+  if constexpr (Lines<N>::YDB > 0 && DT == 0) {
+    if (!env.no_ydb) return launch_y_db<DT, N>(a, s, env, g);
+  }
+  return launch_y<DT, N, YMODE_STEP>(a, s, env, g);
 }
 
 #define SPGPE_DEFINE_LAUNCHERS(N_)                                                               \
-  cudaError_t launch_pass_x_##N_(int dt, int mode, const PassXArgs& a, int ny, cudaStream_t s, int* g) { \
+  cudaError_t launch_pass_x_##N_(int dt, int mode, const PassXArgs& a, int ny, cudaStream_t s, \
+                                 const LaunchEnv& env, int* g) { \
     if (dt == 0) {                                                                               \
       switch (mode) {                                                                            \
-        case MODE_PRO: return launch_x<0, N_, MODE_PRO>(a, ny, s, g);                               \
-        case MODE_MID: return launch_x<0, N_, MODE_MID>(a, ny, s, g);                               \
-        case MODE_EPI: return launch_x<0, N_, MODE_EPI>(a, ny, s, g);                               \
-        default: return launch_x<0, N_, MODE_FWD>(a, ny, s, g);                                     \
+        case MODE_PRO: return launch_x<0, N_, MODE_PRO>(a, ny, s, env, g);                               \
+        case MODE_MID: return launch_x<0, N_, MODE_MID>(a, ny, s, env, g);                               \
+        case MODE_EPI: return launch_x<0, N_, MODE_EPI>(a, ny, s, env, g);                               \
+        default: return launch_x<0, N_, MODE_FWD>(a, ny, s, env, g);                                     \
       }                                                                                          \
     }                                                                                            \
     switch (mode) {                                                                              \
-      case MODE_PRO: return launch_x<1, N_, MODE_PRO>(a, ny, s, g);                                 \
-      case MODE_MID: return launch_x<1, N_, MODE_MID>(a, ny, s, g);                                 \
-      case MODE_EPI: return launch_x<1, N_, MODE_EPI>(a, ny, s, g);                                 \
-      default: return launch_x<1, N_, MODE_FWD>(a, ny, s, g);                                       \
+      case MODE_PRO: return launch_x<1, N_, MODE_PRO>(a, ny, s, env, g);                                 \
+      case MODE_MID: return launch_x<1, N_, MODE_MID>(a, ny, s, env, g);                                 \
+      case MODE_EPI: return launch_x<1, N_, MODE_EPI>(a, ny, s, env, g);                                 \
+      default: return launch_x<1, N_, MODE_FWD>(a, ny, s, env, g);                                       \
     }                                                                                            \
   }                                                                                              \
-  cudaError_t launch_pass_y_##N_(int dt, int ymode, const PassYArgs& a, cudaStream_t s, int* g) { \
+  cudaError_t launch_pass_y_##N_(int dt, int ymode, const PassYArgs& a, cudaStream_t s, \
+                                 const LaunchEnv& env, int* g) { \
     if (dt == 0) {                                                                               \
       switch (ymode) {                                                                           \
-        case YMODE_STEP: return launch_y_step<0, N_>(a, s, g);                            \
-        case YMODE_ENERGY: return launch_y<0, N_, YMODE_ENERGY>(a, s, g);                        \
-        case YMODE_FWDONLY: return launch_y<0, N_, YMODE_FWDONLY>(a, s, g);                      \
-        default: return launch_y<0, N_, YMODE_INVONLY>(a, s, g);                                 \
+        case YMODE_STEP: return launch_y_step<0, N_>(a, s, env, g);                            \
+        case YMODE_ENERGY: return launch_y<0, N_, YMODE_ENERGY>(a, s, env, g);                        \
+        case YMODE_FWDONLY: return launch_y<0, N_, YMODE_FWDONLY>(a, s, env, g);                      \
+        default: return launch_y<0, N_, YMODE_INVONLY>(a, s, env, g);                                 \
       }                                                                                          \
     }                                                                                            \
     switch (ymode) {                                                                             \
-      case YMODE_STEP: return launch_y_step<1, N_>(a, s, g);                              \
-      case YMODE_ENERGY: return launch_y<1, N_, YMODE_ENERGY>(a, s, g);                          \
-      case YMODE_FWDONLY: return launch_y<1, N_, YMODE_FWDONLY>(a, s, g);                        \
-      default: return launch_y<1, N_, YMODE_INVONLY>(a, s, g);                                   \
+      case YMODE_STEP: return launch_y_step<1, N_>(a, s, env, g);                              \
+      case YMODE_ENERGY: return launch_y<1, N_, YMODE_ENERGY>(a, s, env, g);                          \
+      case YMODE_FWDONLY: return launch_y<1, N_, YMODE_FWDONLY>(a, s, env, g);                        \
+      default: return launch_y<1, N_, YMODE_INVONLY>(a, s, env, g);                                   \
     }                                                                                            \
   }
 

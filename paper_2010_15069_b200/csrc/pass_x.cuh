@@ -4,12 +4,13 @@
 // One CTA handles LINES rows; a team of 2*T threads (T = NX/16) owns one row, thread (t, c) holding 16 points of
 // component c.  Lane pairs (c = 0, 1) sit next to each other so that a pair reads/writes one 32-byte point.
 //
-//   MODE_PRO : psi(x) -> [scale] -> R(tau) -> F_x -> * ex_c(k_x) -> psi^(k_x)          (first half of a step)
-//   MODE_MID : psi^(k_x) -> F_x^-1 -> R(tau) R(tau) -> F_x -> * ex_c(k_x) -> psi^(k_x)  (real time, steps n | n+1)
+//   MODE_PRO : psi(x) -> [scale] -> R(tau) -> F_x -> psi^(k_x)                          (first half of a step)
+//   MODE_MID : psi^(k_x) -> F_x^-1 -> R(tau) R(tau) -> F_x -> psi^(k_x)                  (real time, steps n | n+1)
 //   MODE_EPI : psi^(k_x) -> F_x^-1 -> R(tau) -> [norm partials] -> psi(x)              (second half of a step)
 //   MODE_FWD : src psi(x) -> F_x -> dst psi^(k_x)                                      (energy only)
 // The two half-steps of MODE_MID are two evaluations with refreshed densities (R-6); only their scalar phases
-// e^{-i a1 tau} e^{-i a2 tau} are merged into one (unit-modulus phases do not change densities).
+// e^{-i a1 tau} e^{-i a2 tau} are merged into one (unit-modulus phases do not change densities).  One exact exception:
+// when g_uu = g_dd = g_ud the two half-steps are evaluated as one step of 2 tau (real_space_tier, BZ0).
 #pragma once
 #include "line_fft.cuh"
 #include "su2.cuh"
@@ -25,7 +26,6 @@ struct PassXArgs {
   const void* Om;
   const void* De;
   const double2* tw;     // twiddles of NX
-  const double2* exk;    // [2][NX] k_x phase in stored order (MODE_PRO, MODE_MID)
   const double* scale;   // [2] per-component factor applied at load (MODE_PRO, imaginary time) or NULL
   double* partial;       // [ny / LINES][2] sum |psi_c|^2 of every row group (MODE_EPI with want_norm)
   double tau;            // half-step size dt/2
@@ -250,6 +250,7 @@ pass_x_kernel(const PassXArgs a) {
   __shared__ double red[2][32];
   __shared__ int next_s[2];  // group this CTA takes next (written by thread 0, double-buffered over iterations)
   int it = 0;
+  TL_DECL(8);
   for (int grp = blockIdx.x; grp < ngroups; ++it) {
     const size_t first_point = (size_t)grp * LINES * NX;  // first point of the CTA's lines (xs = 1)
     const size_t lbase = line_base(grp * LINES + line);
@@ -265,15 +266,24 @@ pass_x_kernel(const PassXArgs a) {
       for (int n = 0; n < 16; ++n) v[n] = mk(v[n].re * s, v[n].im * s);
     }
     __syncthreads();  // every thread has taken its staged values: the buffers may be overwritten
-    if (MODE == MODE_MID || MODE == MODE_EPI) line_fft_inv<NX>(buf, twS, t, c, v, flip);
-
-    if (MODE != MODE_FWD) {
-      // the exchange buffer is idle during the real-space part: it holds the field rows meanwhile
+    TL_MARK(0);
+    // The exchange buffer is idle during the real-space part: it holds the field rows meanwhile.  Their copy starts
+    // as soon as every warp has done its last read of the line buffers (the loads of the inverse transform's last
+    // radix-16 stage), so it runs under that stage's twiddles and butterflies.
+    auto fields_hook = [&]() {
       __syncthreads();
       stage_fields<DT, NX, LINES, XS>(smem, a, first_point, grp * LINES, tid);
+    };
+    if (MODE == MODE_MID || MODE == MODE_EPI) line_fft_inv<NX>(buf, twS, t, c, v, flip, fields_hook);
+    TL_MARK(1);
+
+    if (MODE != MODE_FWD) {
+      if (MODE == MODE_PRO) fields_hook();
       cp_async_wait_all();
       __syncthreads();
+      TL_MARK(2);
       real_space<DT, NX, LINES, MODE>(v, a, smem, line, t, c, lc, sm, so);
+      TL_MARK(3);
       if (MODE == MODE_EPI && tid == 0) next_s[it & 1] = nxt_req;
       if (MODE == MODE_EPI && a.want_norm) {
         // norm partials of this row group, one slot per group: the sums do not depend on which CTA took the group,
@@ -309,21 +319,17 @@ pass_x_kernel(const PassXArgs a) {
       if (tid == 0) next_s[it & 1] = nxt_req;
       __syncthreads();  // the last exchange has been read by every warp: the line buffers are free
       nxt_grp = next_s[it & 1];
+      TL_MARK(4);
       if (nxt_grp < ngroups) issue_loads(nxt_grp);
       dft_last<-1, P::RL>(v);
-      // k_x phase table: one base per thread, pinned behind the last butterfly (late_zero)
-      const double2* ex = a.exk + c * NX + t + late_zero(v[0].re);
+      TL_MARK(5);
+      // the k_x phase of the k-space factor is applied by the column pass (one table value per thread there)
 #pragma unroll
       for (int g = 0; g < P::G; ++g)
 #pragma unroll
         for (int s = 0; s < P::RL; ++s) {
           const int off = g * T + (NX / P::RL) * s;
-          cplx o = v[g * P::RL + s];
-          if (MODE != MODE_FWD) {
-            double2 e = __ldg(ex + off);
-            o = cmul(o, mk(e.x, e.y));
-          }
-          St::st(a.dst, (lbase + (size_t)(t + off) * S) * 2 + c, o);
+          St::st(a.dst, (lbase + (size_t)(t + off) * S) * 2 + c, v[g * P::RL + s]);
         }
     }
     if (MODE != MODE_FWD && S == 1 && tid == 0 && nxt_grp < ngroups) {  // field rows of the next group: into L2
@@ -332,8 +338,11 @@ pass_x_kernel(const PassXArgs a) {
       if (a.Om) prefetch_l2_bulk(reinterpret_cast<const real*>(a.Om) + nxt, LINES * NX * (unsigned)sizeof(real));
       if (a.De) prefetch_l2_bulk(reinterpret_cast<const real*>(a.De) + nxt, LINES * NX * (unsigned)sizeof(real));
     }
+    TL_MARK(6);
+    TL_TILE();
     grp = nxt_grp;
   }
+  if (MODE == MODE_MID) TL_DUMP("xmid wait+stage|inv|fields|real|fwd|issue+last|ex+store", 7);
   if (MODE == MODE_EPI) {
     // imaginary time (a6): the CTA that finishes last turns the per-group norm partials into the rescale factors
     // of the next step (fixed summation order), so no separate kernel is needed
@@ -359,11 +368,12 @@ pass_x_kernel(const PassXArgs a) {
           for (int i = 0; i < NTHR / 32; ++i) { nu += red[0][i]; nd += red[1][i]; }
           nu *= a.cell;
           nd *= a.cell;
+          // a component (or state) of zero norm keeps scale 1 and stays zero instead of turning into NaN (0/0)
           if (a.norm_mode == 0) {
-            a.scale_out[0] = sqrt(a.target[0] / nu);
-            a.scale_out[1] = sqrt(a.target[1] / nd);
+            a.scale_out[0] = nu > 0.0 ? sqrt(a.target[0] / nu) : 1.0;
+            a.scale_out[1] = nd > 0.0 ? sqrt(a.target[1] / nd) : 1.0;
           } else {
-            a.scale_out[0] = a.scale_out[1] = sqrt((a.target[0] + a.target[1]) / (nu + nd));
+            a.scale_out[0] = a.scale_out[1] = (nu + nd) > 0.0 ? sqrt((a.target[0] + a.target[1]) / (nu + nd)) : 1.0;
           }
         }
       }

@@ -1,12 +1,13 @@
 // pass_y.cuh -- the column pass: y-direction forward transform, k-space phase, inverse transform
 // (SURVEY.md 8(a) rows a2/a4 (y part) and a3; include/spgpe.h).  The k-space factor
-// exp(-i K_c dt) is separable: the k_x factor is applied at the end of the row pass, here only
-// ey(k_y) = exp(-i k_y^2 dt / 2) / (nx ny) (imaginary time: the decaying real factor).
+// exp(-i K_c dt) is separable into ex_c(k_x) ey(k_y), ey(k_y) = exp(-i k_y^2 dt / 2) / (nx ny) (imaginary time: the
+// decaying real factors).  Both are applied here: ey from a per-thread table, ex_c(k_x) as ONE value per thread and
+// tile, since a thread's 16 points share their column (in the row pass it would take 16 table loads per thread).
 //
 // One CTA handles LINES adjacent columns; thread index = c + 2*(line + LINES*t), so that a warp-wide access
 // covers LINES*32 contiguous bytes in each of 16/LINES rows.
 //
-//   YMODE_STEP   : psi^(k_x, y) -> F_y -> * ey(k_y) -> F_y^-1 -> psi^(k_x, y)            (in place)
+//   YMODE_STEP   : psi^(k_x, y) -> F_y -> * ex_c(k_x) ey(k_y) -> F_y^-1 -> psi^(k_x, y)  (in place)
 //   YMODE_ENERGY : psi^(k_x, y) -> F_y -> sum (Kx_c(k_x) + Ky(k_y)) |psi^|^2 -> partial[CTA]
 //   YMODE_FWDONLY: psi^(k_x, y) -> F_y -> psi^(k_x, k_y) in stored order          (split transforms, api.cu)
 //   YMODE_INVONLY: psi^(k_x, k_y) in stored order -> F_y^-1 -> psi^(k_x, y)
@@ -23,6 +24,7 @@ struct PassYArgs {
   void* psi;            // [NY][nx][2]
   const double2* tw;    // twiddles of NY
   const double2* eyk;   // [NY] k_y phase in stored order (YMODE_STEP)
+  const double2* exk;   // [2][nx] k_x phase in the row pass's stored order (YMODE_STEP), or NULL (none applied here)
   const double* Kx;     // [2][nx] (k_x +- k_L)^2/2 in the row pass's stored order (YMODE_ENERGY)
   const double* Ky;     // [NY] k_y^2/2 in stored order (YMODE_ENERGY)
   double* partial;      // [gridDim.x] sum over this CTA's columns (YMODE_ENERGY)
@@ -43,21 +45,22 @@ struct YLayout {
 
 // dynamic shared memory of the column pass: LINES padded line buffers, the twiddle table, and (YMODE_STEP, when
 // it fits in 227 KB) the k_y phase table
-template <int NY, int LINES>
+// EYG: the k_y phase table stays in global memory (read through L1/L2) so that two CTAs fit one SM
+template <int NY, int LINES, bool EYG = false>
 struct YSmem {
   static constexpr int EBUF = LINES * YLayout<NY, LINES>::LINE_PTS * 2;  // double2 elements
   static constexpr int TW = tw_total<NY>();
-  static constexpr bool EY_SMEM = (size_t)(EBUF + TW + NY) * 16 <= 227u * 1024u;
+  static constexpr bool EY_SMEM = !EYG && (size_t)(EBUF + TW + NY) * 16 <= 227u * 1024u;
   static constexpr size_t BYTES = (size_t)(EBUF + TW + (EY_SMEM ? NY : 0)) * 16;
 };
 
 // Persistent: CTA b handles the column groups b, b + gridDim.x, ...
-template <int DT, int NY, int LINES, int YMODE>
+template <int DT, int NY, int LINES, int YMODE, bool EYG = false>
 __global__ void __launch_bounds__(LINES * (NY / 8), (LINES * (NY / 8) <= 256) ? 2 : 1)
 pass_y_kernel(const __grid_constant__ PassYArgs a) {
   typedef Plan<NY> P;
   typedef Store<DT> St;
-  typedef YSmem<NY, LINES> SM;
+  typedef YSmem<NY, LINES, EYG> SM;
   extern __shared__ __align__(128) double2 smem[];
   constexpr int T = P::T;
   constexpr int NTHR = LINES * (NY / 8);
@@ -100,7 +103,11 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
     mbar_init(&mbar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  pdl_wait();  // psi, the phase table and the work counter belong to the preceding kernels
+  // psi and the work counter belong to the preceding kernel.  The tables copied above do not: the twiddles are
+  // written at spgpe_create, and the k_y phase table by aux_phase_tables, an ordinary (non-programmatic) launch that
+  // has completed before the row pass in front of this kernel could start; this kernel can only become resident
+  // after that row pass has started, so the table is complete whenever the prologue runs.
+  pdl_wait();
   if (tid == 0 && (int)blockIdx.x < ngroups) issue_loads(blockIdx.x);
   cp_async_wait_all();
   __syncthreads();  // tables and the barrier are visible to every thread
@@ -110,6 +117,9 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
   for (int grp = blockIdx.x; grp < ngroups; ++it) {
     const size_t col = (size_t)grp * LINES + line;
     const size_t e0 = ((size_t)t * nx + col) * 2 + c;  // element (row t, column col, component c)
+    // k_x phase of this column and component (see pass_y_db_kernel); requested now, used after the forward transform
+    double2 exv = make_double2(1.0, 0.0);
+    if (YMODE == YMODE_STEP && a.exk != nullptr) exv = __ldg(a.exk + (size_t)c * nx + col);
     // the next group is requested now and published before the last barrier of this iteration (latency hidden)
     int nxt_req = 0;
     if (tid == 0) {
@@ -143,7 +153,7 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
         for (int s = 0; s < P::RL; ++s) {
           const int pos = (t + g * T) + (NY / P::RL) * s;
           double2 f = SM::EY_SMEM ? ey[pos] : __ldg(ey + pos + late_zero(v[g * P::RL + s].re));
-          v[g * P::RL + s] = cmul(v[g * P::RL + s], mk(f.x, f.y));
+          v[g * P::RL + s] = cmul(cmul(v[g * P::RL + s], mk(f.x, f.y)), mk(exv.x, exv.y));
         }
       }
       // after the last read of the line buffers the next group's transfer starts under the last butterflies
@@ -202,35 +212,41 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
 }
 
 // ---- double-buffered variant of YMODE_STEP ------------------------------------------------------------------------
-// One 256-thread CTA per SM works on tiles of LINES columns with a staging buffer next to the line buffers: the TMA
-// load of the next tile is issued as soon as the current one has been taken out of the staging buffer, a whole tile
-// period ahead, and the results leave through the (then idle) line buffers with a TMA store.  No warp ever issues a
-// global load or store, and the DRAM traffic is spread over the whole period instead of coming in bursts between
-// the transforms.
+// One 256-thread CTA per SM works on tiles of LINES columns with three buffers: the line buffers (exchanges of the
+// transforms), a staging buffer (the TMA load of the next tile is issued as soon as the current one has been taken
+// out of it, a whole tile period ahead) and an output buffer (the results leave with a TMA store that has a whole
+// tile period to drain).  No warp ever issues a global load or store of psi, and the DRAM traffic is spread over the
+// whole period instead of coming in bursts between the transforms.  With 256 threads per SM the kernel has registers
+// to spare: the k_y phases of a thread's 16 stored positions and its 15 stage-1 twiddles live in registers (loaded
+// once from global memory), so shared memory holds only the twiddles of the later stages.
 template <int NY, int LINES>
 struct YSmemDB {
   static constexpr int EBUF = LINES * YLayout<NY, LINES>::LINE_PTS * 2;  // double2 elements
-  static constexpr int STG = NY * LINES * 2;                             // staging, in double2 elements (c128)
-  static constexpr int TW = tw_total<NY>();
-  static constexpr size_t BYTES = (size_t)(EBUF + STG + TW + NY) * 16;
+  static constexpr int STG = NY * LINES * 2;                             // staging / output, in double2 elements (c128)
+  static constexpr int TW2 = tw_total<NY>() - tw_offset<NY>(2);          // twiddles of stages >= 2
+  static constexpr size_t BYTES = (size_t)(EBUF + 2 * STG + TW2) * 16;
   static constexpr bool FITS = BYTES <= 227u * 1024u;
 };
 
-// CTA-wide exchanges; before the first one of a tile the line buffers must have been released by the TMA store of
-// the previous tile (thread 0 waits for it, the barrier tells the others)
-struct StoreDrainSync {
+// CTA-wide exchanges, stage-1 twiddles in registers.  A three-stage transform has exactly one CTA-wide barrier (the
+// exchange after stage 1); the kernel hangs its own hand-overs on it instead of adding barriers: with mode = 1
+// thread 0 runs `after` behind the next barrier, with mode = 2 it runs `before` ahead of it (then mode returns to 0).
+template <typename Before, typename After>
+struct RegTwSync {
   static constexpr bool REG_TW1 = true;
-  mutable bool pending;
+  double2 tw1[15];  // the thread's stage-1 twiddles
+  Before before;
+  After after;
   int tid;
-  double2 tw1[15];  // the thread's stage-1 twiddles (this kernel has registers to spare: 256 threads per SM)
-  __device__ __forceinline__ void sync() const { __syncthreads(); }
-  __device__ __forceinline__ void acquire() const {
-    if (pending) {
-      if (tid == 0) tma_store_wait_read();
-      __syncthreads();
-      pending = false;
-    }
+  mutable int mode;
+  __device__ __forceinline__ RegTwSync(Before b, After a_, int tid_) : before(b), after(a_), tid(tid_), mode(0) {}
+  __device__ __forceinline__ void sync() const {
+    if (mode == 2 && tid == 0) before();
+    __syncthreads();
+    if (mode == 1 && tid == 0) after();
+    mode = 0;
   }
+  __device__ __forceinline__ void acquire() const {}
   __device__ __forceinline__ void release() const {}
 };
 
@@ -240,6 +256,7 @@ __global__ void __launch_bounds__(LINES * (NY / 8), 1) pass_y_db_kernel(const __
   typedef Store<DT> St;
   typedef typename St::elem elem;
   typedef YSmemDB<NY, LINES> SM;
+  static_assert(P::NS == 3, "the double-buffered column pass is built for three-stage plans");
   extern __shared__ __align__(128) double2 smem[];
   constexpr int T = P::T;
   constexpr int NTHR = LINES * (NY / 8);
@@ -250,15 +267,14 @@ __global__ void __launch_bounds__(LINES * (NY / 8), 1) pass_y_db_kernel(const __
   const int line = (tid >> 1) % LINES;
   const int t = (tid >> 1) / LINES;
   double2* buf = smem + (size_t)line * (YLayout<NY, LINES>::LINE_PTS * 2);
-  elem* out = reinterpret_cast<elem*>(smem);             // results leave through the line buffers
-  elem* stg = reinterpret_cast<elem*>(smem + SM::EBUF);  // the next tile arrives here
-  double2* twS = smem + SM::EBUF + SM::STG;
-  double2* eyS = twS + SM::TW;
+  elem* stg = reinterpret_cast<elem*>(smem + SM::EBUF);            // the next tile arrives here
+  elem* out = reinterpret_cast<elem*>(smem + SM::EBUF + SM::STG);  // results leave from here
+  double2* tw2S = smem + SM::EBUF + 2 * SM::STG;
+  const double2* twS = tw2S - tw_offset<NY>(2);  // table base as line_fft.cuh indexes it; stage 1 is never read
   __shared__ __align__(8) unsigned long long mbar;
   __shared__ int next_s[2];
   pdl_launch_dependents();
-  copy_table_async(twS, a.tw, SM::TW, tid, NTHR);
-  copy_table_async(eyS, a.eyk, NY, tid, NTHR);
+  copy_table_async(tw2S, a.tw + tw_offset<NY>(2), SM::TW2, tid, NTHR);
   const int ngroups = a.nx / LINES;
   auto issue_loads = [&](int grp) {  // thread 0 only
     fence_proxy_async();
@@ -267,60 +283,86 @@ __global__ void __launch_bounds__(LINES * (NY / 8), 1) pass_y_db_kernel(const __
     for (int b = 0; b < NY / BR; ++b)
       tma_load_2d(stg + (size_t)b * BR * LINES * 2, &a.tmap_db, grp * LINES * 4, b * BR, &mbar);
   };
+  // Work distribution: the tile of iteration it+1 is in `nxt`, fetched (atomic) one iteration ahead by thread 0 so
+  // that its latency never sits in front of a barrier; published to the other threads through next_s.
+  int nxt = 0, it = 0;
+  // hand-overs on the transforms' own barriers (thread 0):
+  //  forward: behind the barrier every thread has taken its values out of the staging buffer -> load the next tile
+  //  inverse: ahead of the barrier the store of the previous tile (issued a period ago) has released the output buffer
+  auto load_next = [&]() {
+    if (nxt < ngroups) {
+      issue_loads(nxt);
+      nxt = sched_next(a.sched);  // consumed in the next iteration
+    } else {
+      nxt = ngroups;
+    }
+  };
+  auto drain_out = [&]() { if (it > 0) tma_store_wait_read(); };
+  // per-thread constants kept in registers for the whole kernel (tables written before any pass kernel started, see
+  // pass_y_kernel): the thread's 15 stage-1 twiddles and the k_y phases of its 16 stored positions
+  RegTwSync<decltype(drain_out), decltype(load_next)> sy(drain_out, load_next, tid);
+#pragma unroll
+  for (int k = 1; k < 16; ++k) sy.tw1[k - 1] = __ldg(a.tw + tw_offset<NY>(1) + (k - 1) * (NY >> 4) + t);
+  double2 eyr[16];
+#pragma unroll
+  for (int g = 0; g < P::G; ++g)
+#pragma unroll
+    for (int s = 0; s < P::RL; ++s) eyr[g * P::RL + s] = __ldg(a.eyk + (t + g * T) + (NY / P::RL) * s);
   if (tid == 0) {
     mbar_init(&mbar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   pdl_wait();
-  if (tid == 0 && (int)blockIdx.x < ngroups) issue_loads(blockIdx.x);
+  if (tid == 0) {
+    if ((int)blockIdx.x < ngroups) issue_loads(blockIdx.x);
+    nxt = sched_next(a.sched);
+  }
   cp_async_wait_all();
   __syncthreads();
-  // per-thread constants kept in registers for the whole kernel: the k_y phases of the thread's 16 stored positions
-  // and its 15 stage-1 twiddles
-  StoreDrainSync sy;
-  sy.tid = tid;
-  sy.pending = false;
-#pragma unroll
-  for (int k = 1; k < 16; ++k) sy.tw1[k - 1] = twS[tw_offset<NY>(1) + (k - 1) * (NY >> 4) + t];
-  double2 eyr[16];
-#pragma unroll
-  for (int g = 0; g < P::G; ++g)
-#pragma unroll
-    for (int s = 0; s < P::RL; ++s) eyr[g * P::RL + s] = eyS[(t + g * T) + (NY / P::RL) * s];
   cplx v[16];
-  int it = 0;
+  TL_DECL(8);
   for (int grp = blockIdx.x; grp < ngroups; ++it) {
-    if (tid == 0) next_s[it & 1] = sched_next(a.sched);
+    // k_x phase of this column and component (applied here and not at the end of the row pass: there it costs
+    // sixteen table loads per thread, here one); requested now, used after the forward transform
+    double2 exv = make_double2(1.0, 0.0);
+    if (a.exk != nullptr) exv = __ldg(a.exk + (size_t)c * a.nx + (size_t)grp * LINES + line);
+    if (tid == 0) next_s[it & 1] = nxt;  // visible to everyone behind the forward transform's barrier
     mbar_wait(&mbar, it & 1);
+    TL_MARK(0);
 #pragma unroll
     for (int n = 0; n < 16; ++n) v[n] = St::cv(stg[((t + n * T) * LINES + line) * 2 + c]);
-    __syncthreads();  // the staging buffer is free; next_s is visible
-    const int nxt_grp = next_s[it & 1];
-    if (tid == 0 && nxt_grp < ngroups) issue_loads(nxt_grp);
-
-    sy.pending = it > 0;  // the first exchange waits for the previous tile's store to drain
+    TL_MARK(1);
+    sy.mode = 1;
     line_fft_fwd<NY>(buf, twS, t, c, v, 0, sy);
+    TL_MARK(2);
 #pragma unroll
     for (int g = 0; g < P::G; ++g)
 #pragma unroll
       for (int s = 0; s < P::RL; ++s) {
         const double2 f = eyr[g * P::RL + s];
-        v[g * P::RL + s] = cmul(v[g * P::RL + s], mk(f.x, f.y));
+        v[g * P::RL + s] = cmul(cmul(v[g * P::RL + s], mk(f.x, f.y)), mk(exv.x, exv.y));
       }
-    auto hook = [&]() { __syncthreads(); };  // every warp has done its last read of the line buffers
-    line_fft_inv<NY>(buf, twS, t, c, v, 0, hook, sy);
+    TL_MARK(3);
+    sy.mode = 2;
+    line_fft_inv<NY>(buf, twS, t, c, v, 0, NoHook(), sy);
+    TL_MARK(4);
+    const int nxt_grp = next_s[it & 1];
 #pragma unroll
     for (int n = 0; n < 16; ++n) out[((t + n * T) * LINES + line) * 2 + c] = St::el(v[n]);
     fence_proxy_async();  // these generic-proxy writes are read by the TMA store
     __syncthreads();
+    TL_MARK(5);
     if (tid == 0) {
 #pragma unroll
       for (int b = 0; b < NY / BR; ++b)
         tma_store_2d(&a.tmap_db, grp * LINES * 4, b * BR, out + (size_t)b * BR * LINES * 2);
       tma_store_commit();
     }
+    TL_MARK(6);
+    TL_TILE();
     grp = nxt_grp;
   }
+  TL_DUMP("ydb wait|stage|fwd|ey|inv|out|store", 7);
   if (tid == 0) {
     tma_store_wait_all();
     sched_finish(a.sched);

@@ -4,7 +4,7 @@
 // ordinary pass kernels; this kernel supplies the radix-2 decimation-in-time step that joins them, applies the
 // k-space phase of the split axes on the joined spectrum and undoes the join:
 //   X[f]     = E[f] + w^f O[f],   X[f + m] = E[f] - w^f O[f],   w = exp(-2 pi i / n),  f = 0..m-1
-//   X <- phase * X                                              (on the split axes only)
+//   X <- phase * X                                              (k_x phase always, k_y phase of a split y axis)
 //   E'[f]    = X[f] + X[f + m],   O'[f]    = conj(w^f) (X[f] - X[f + m])          (unnormalised, like the passes)
 // E and O sit interleaved in memory: sub-line p of the x axis occupies the points x = 2 pos + p, sub-line p of the
 // y axis the rows y = 2 pos + p, pos = stored position of the sub-transform.  One thread owns the SX x SY block of
@@ -67,7 +67,7 @@ __global__ void __launch_bounds__(256) split_kernel(const SplitArgs a) {
           }
       continue;
     }
-    if (SX == 2) {
+    {  // k_x phase: by true frequency along a split x axis, by stored position (fx = px, i = 0) along an unsplit one
 #pragma unroll
       for (int j = 0; j < SY; ++j)
 #pragma unroll
