@@ -36,7 +36,7 @@ struct spgpe_ctx {
   int tab_imag;
   bool tab_valid;
   double *partial, *scale, *target, *dout;
-  CUtensorMap tmap_psi, tmap_scratch, tmap_psi_db;  // column-pass tensor maps of psi and of the energy scratch buffer
+  CUtensorMap tmap_psi, tmap_scratch, tmap_psi_db, tmap_psi_duo;  // column-pass tensor maps of psi / the energy scratch buffer
   int* sched;    // [4] work counters of the persistent kernels: row pass [0..1], column pass [2..3]
   double2 *wcx, *wcy;         // split axes: join twiddles
   int *fpx, *fpy;             // split axes: true frequency of a sub-transform position
@@ -111,7 +111,7 @@ static int cuda_fail(cudaError_t e) {
 
 // Tensor map of a psi-shaped buffer for the column pass (pass_y.cuh): 2-D [ny rows][4 nx reals], box of
 // min(ny, 256) rows x 4 * lines reals.  The driver entry point is looked up at run time (no libcuda link).
-static cudaError_t make_col_tmap(const spgpe_ctx* h, void* base, int lines, CUtensorMap* out) {
+static cudaError_t make_col_tmap(const spgpe_ctx* h, void* base, int lines, CUtensorMap* out, int rows = 0) {
   // looked up once per process (the driver entry point is the same for every device); C++11 makes the
   // initialisation of a function-local static thread-safe
   static const PFN_cuTensorMapEncodeTiled_v12000 encode = []() -> PFN_cuTensorMapEncodeTiled_v12000 {
@@ -126,7 +126,8 @@ static cudaError_t make_col_tmap(const spgpe_ctx* h, void* base, int lines, CUte
   // a split y axis is seen as my rows of sy * nx points: row r of that view holds the rows sy * r + p of the grid
   const cuuint64_t gdim[2] = {(cuuint64_t)h->nx * h->sy * 4, (cuuint64_t)h->my};
   const cuuint64_t gstride[1] = {(cuuint64_t)h->nx * h->sy * 4 * rsz};
-  const cuuint32_t box[2] = {(cuuint32_t)lines * 4, (cuuint32_t)(h->my < 256 ? h->my : 256)};
+  if (rows <= 0) rows = h->my < 256 ? h->my : 256;
+  const cuuint32_t box[2] = {(cuuint32_t)lines * 4, (cuuint32_t)rows};
   const cuuint32_t estr[2] = {1, 1};
   CUresult r = encode(out, h->dt == SPGPE_C128 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
                       base, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -226,6 +227,7 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
   h->env.device = dev;
   h->env.ctas_per_sm = env_int("SPGPE_DEBUG_CTAS_PER_SM");
   h->env.no_ydb = env_int("SPGPE_DEBUG_NO_YDB");
+  h->env.xdbg = env_int("SPGPE_DEBUG_X");
   int split_min = env_int("SPGPE_DEBUG_SPLIT_MIN");
   if (split_min < 128) split_min = 8192;
   h->sx = split_of(nx, split_min); h->sy = split_of(ny, split_min); h->mx = nx / h->sx; h->my = ny / h->sy;
@@ -309,6 +311,7 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
   }
   if (e == cudaSuccess) e = make_col_tmap(h, h->psi, plan_lines_y(h->my), &h->tmap_psi);
   if (e == cudaSuccess && plan_lines_ydb(h->my) > 0) e = make_col_tmap(h, h->psi, plan_lines_ydb(h->my), &h->tmap_psi_db);
+  if (e == cudaSuccess && plan_has_duo(h->my) && h->dt == SPGPE_C128) e = make_col_tmap(h, h->psi, 1, &h->tmap_psi_duo, h->my / 16);
   if (e != cudaSuccess) {
     spgpe_destroy(h);
     return e == cudaErrorMemoryAllocation ? SPGPE_ERR_NO_MEMORY : cuda_fail(e);
@@ -458,13 +461,13 @@ extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
   xa.src = h->psi; xa.dst = h->psi; xa.V = h->V; xa.Om = h->Om; xa.De = h->De;
   xa.tw = h->tw_x; xa.scale = nullptr; xa.partial = h->partial;
   xa.tau = 0.5 * dt; xa.hc = h->hc; xa.imag = imag; xa.want_norm = imag; xa.ny = h->ny * h->sx; xa.xs = h->sx;
-  xa.fmax = h->fmax; xa.sched = h->sched;
+  xa.fmax = h->fmax; xa.sched = h->sched; xa.dbg = h->env.xdbg;
   xa.target = h->target; xa.scale_out = h->scale; xa.cell = (h->Lx / h->nx) * (h->Ly / h->ny); xa.norm_mode = h->p.norm_mode;
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
   ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx * h->sy;
   // the k_x phase rides on the column pass unless a split axis sends the k-space phases to the join kernel
-  ya.exk = (h->sx == 1 && h->sy == 1) ? h->exk : nullptr; ya.sched = h->sched + 2; ya.tmap = h->tmap_psi; ya.tmap_db = h->tmap_psi_db;
+  ya.exk = (h->sx == 1 && h->sy == 1) ? h->exk : nullptr; ya.sched = h->sched + 2; ya.tmap = h->tmap_psi; ya.tmap_db = h->tmap_psi_db; ya.tmap_duo = h->tmap_psi_duo;
   if (!imag) {
     CK(dispatch_x(h, MODE_PRO, xa));
     for (int s = 1; s <= n; ++s) {

@@ -34,6 +34,7 @@ struct LaunchEnv {
   int device;        // CUDA device ordinal of the handle
   int ctas_per_sm;   // SPGPE_DEBUG_CTAS_PER_SM: cap on resident CTAs per SM of the persistent kernels (0: none)
   int no_ydb;        // SPGPE_DEBUG_NO_YDB: column pass without the double-buffered kernel
+  int xdbg;          // SPGPE_DEBUG_X: experiment switches of the row pass
 };
 
 struct cplx {
@@ -117,6 +118,8 @@ template <> struct Store<1> {
   static __device__ __forceinline__ float2 el(cplx c) { return make_float2((float)c.re, (float)c.im); }
 };
 
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
 // ---- asynchronous copies ------------------------------------------------------------------------------------
 // 16-byte global -> shared copy that bypasses registers (LDGSTS); completion through cp_async_wait_all
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
@@ -137,13 +140,36 @@ __device__ __forceinline__ void cp_async_real(float* smem_dst, const float* gsrc
 __device__ __forceinline__ void cp_async_elem(double2* smem_dst, const double2* gsrc) { cp_async16(smem_dst, gsrc); }
 __device__ __forceinline__ void cp_async_elem(float2* smem_dst, const float2* gsrc) { cp_async8(smem_dst, gsrc); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+// 1-D bulk copy global -> shared memory (one instruction for a whole row; bytes a multiple of 16, both addresses
+// 16-byte aligned), completion on bar
+__device__ __forceinline__ void bulk_load_1d(void* smem_dst, const void* gsrc, unsigned bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(smem_dst)),
+               "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+// L2 eviction policy for data that is read once per pass (the fields): evict first, so that the streams do not
+// push the order parameter, which the next pass reads again, out of L2
+__device__ __forceinline__ unsigned long long l2_policy_evict_first() {
+  unsigned long long p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+// bulk_load_1d with an L2 cache policy
+__device__ __forceinline__ void bulk_load_1d_hint(void* smem_dst, const void* gsrc, unsigned bytes,
+                                                  unsigned long long* bar, unsigned long long policy) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+          smem_u32(smem_dst)),
+      "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+      : "memory");
+}
 // ask L2 to fetch `bytes` (multiple of 16) starting at the 16-byte aligned address p; no registers, no scoreboard
 __device__ __forceinline__ void prefetch_l2_bulk(const void* p, unsigned bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
 // ---- TMA (cp.async.bulk.tensor) and mbarrier, raw PTX ----------------------------------------------------------
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }

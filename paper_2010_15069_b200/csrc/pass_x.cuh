@@ -40,16 +40,19 @@ struct PassXArgs {
   double cell;           // dx dy
   int norm_mode;         // SPGPE_NORM_PER_COMPONENT | SPGPE_NORM_TOTAL
   const double* fmax;    // [3] device: max |V|, max |Omega|, max |delta| over the grid (tier bounds)
+  int dbg;               // experiment switches (bit 0: psi rows by bulk copy, 1: field rows by bulk copy, 2: early L2 prefetch)
 };
 
 __device__ __forceinline__ double shfl_xor_d(double x, int m) { return __shfl_xor_sync(0xffffffffu, x, m); }
 __device__ __forceinline__ cplx shfl_xor_c(cplx a, int m) { return mk(shfl_xor_d(a.re, m), shfl_xor_d(a.im, m)); }
 
-// Copy the three field rows of this CTA's LINES rows into shared memory ([field][line][x], working precision),
-// 16 bytes per cp.async; a NULL field is filled with zeros.  Every thread of the CTA takes part.
+// Copy the three field rows of this CTA's LINES rows into shared memory ([field][line][x], working precision); a NULL
+// field is filled with zeros.  Every thread of the CTA takes part.  Rows (XS == 1) are contiguous: thread 0 issues one
+// bulk copy per field (completion on `bar`, evict-first in L2: the fields are read once per pass and must not push
+// the order parameter out); the strided lines of a split axis take one cp.async per real.
 template <int DT, int NX, int LINES, int XS>
 __device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, size_t first_point, int first_line,
-                                             int tid) {
+                                             int tid, unsigned long long* bar, bool fbulk) {
   typedef typename Store<DT>::real real;
   constexpr int FIELD_BYTES = LINES * NX * (int)sizeof(real);
   constexpr int NCH = FIELD_BYTES / 16;
@@ -67,7 +70,7 @@ __device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, siz
         else dst[k] = (real)0;
       }
     }
-  } else {
+  } else if (!fbulk) {
 #pragma unroll
     for (int f = 0; f < 3; ++f) {
       char* dst = reinterpret_cast<char*>(fbuf) + f * FIELD_BYTES;
@@ -76,6 +79,27 @@ __device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, siz
 #pragma unroll
         for (int k = tid; k < NCH; k += NTHR) cp_async16(dst + k * 16, g + k * 16);
       } else {
+#pragma unroll
+        for (int k = tid; k < NCH; k += NTHR)
+          *reinterpret_cast<float4*>(dst + k * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+    }
+  } else {
+    if (tid == 0) {
+      const unsigned long long policy = l2_policy_evict_first();
+      const unsigned n = (src[0] != nullptr) + (src[1] != nullptr) + (src[2] != nullptr);
+      fence_proxy_async();
+      mbar_expect_tx(bar, n * (unsigned)FIELD_BYTES);  // n == 0: the phase completes at once
+#pragma unroll
+      for (int f = 0; f < 3; ++f)
+        if (src[f] != nullptr)
+          bulk_load_1d_hint(reinterpret_cast<char*>(fbuf) + f * FIELD_BYTES,
+                            reinterpret_cast<const char*>(src[f]) + first_point * sizeof(real), FIELD_BYTES, bar, policy);
+    }
+#pragma unroll
+    for (int f = 0; f < 3; ++f) {
+      if (src[f] == nullptr) {
+        char* dst = reinterpret_cast<char*>(fbuf) + f * FIELD_BYTES;
 #pragma unroll
         for (int k = tid; k < NCH; k += NTHR)
           *reinterpret_cast<float4*>(dst + k * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -220,32 +244,81 @@ pass_x_kernel(const PassXArgs a) {
   double2* twS = smem + XSmem<NX, LINES>::EBUF;
   pdl_launch_dependents();
   copy_table_async(twS, a.tw, tw_total<NX>(), tid, NTHR);  // completes with the first cp_async_wait_all below
-  pdl_wait();
 
-  // The psi rows of a group travel global -> shared memory asynchronously (cp.async into the line buffers, which
-  // are idle at that time: slot (n, tid) holds register n of thread tid), issued one group ahead so that the
-  // transfer runs under the tail of the previous group instead of stalling the CTA at the head of this one.
+  // The psi rows of a group travel global -> shared memory asynchronously into the line buffers, which are idle at
+  // that time, one group ahead, so that the transfer runs under the tail of the previous group.  Rows (XS == 1) are
+  // contiguous: ONE bulk copy (cp.async.bulk, mbarrier completion) moves the LINES rows of a group and they land in
+  // memory order [line][x][c].  The interleaved half rows of a split axis (XS == 2) go through per-thread cp.async,
+  // slot (n, tid) holding register n of thread tid.
   elem* stg = reinterpret_cast<elem*>(smem);
-  // point index of position 0 of line L: lines are rows (xs = 1) or the even / odd points of a row (xs = 2)
   constexpr int S = XS;  // == a.xs
+  const bool BULK = (XS == 1) && (a.dbg & 1);
+  const bool FBULK = (XS == 1) && (a.dbg & 2);
+  constexpr unsigned GROUP_BYTES = (unsigned)LINES * NX * 2 * (unsigned)sizeof(elem);
+  __shared__ __align__(8) unsigned long long full, ffull;  // psi rows landed / field rows landed
+  // point index of position 0 of line L: lines are rows (xs = 1) or the even / odd points of a row (xs = 2)
   auto line_base = [&](int L) { return (size_t)(L / S) * NX * S + (size_t)(L % S); };
   auto issue_loads = [&](int grp) {
-    const size_t lb = line_base(grp * LINES + line);
     const elem* src = reinterpret_cast<const elem*>(a.src);
-    if (MODE == MODE_PRO || MODE == MODE_FWD) {
-#pragma unroll
-      for (int n = 0; n < 16; ++n)
-        cp_async_elem(stg + n * NTHR + tid, src + (lb + (size_t)(t + ((n + 8 * c) & 15) * T) * S) * 2 + c);
+    if (BULK) {
+      if (tid == 0) {
+        fence_proxy_async();  // the line buffers were last touched through the generic proxy
+        mbar_expect_tx(&full, GROUP_BYTES);
+        bulk_load_1d(stg, src + (size_t)grp * LINES * NX * 2, GROUP_BYTES, &full);
+      }
     } else {
+      const size_t lb = line_base(grp * LINES + line);
+      if (MODE == MODE_PRO || MODE == MODE_FWD) {
 #pragma unroll
-      for (int g = 0; g < P::G; ++g)
+        for (int n = 0; n < 16; ++n)
+          cp_async_elem(stg + n * NTHR + tid, src + (lb + (size_t)(t + ((n + 8 * c) & 15) * T) * S) * 2 + c);
+      } else {
 #pragma unroll
-        for (int s = 0; s < P::RL; ++s)
-          cp_async_elem(stg + (g * P::RL + s) * NTHR + tid,
-                        src + (lb + (size_t)((t + g * T) + (NX / P::RL) * s) * S) * 2 + c);
+        for (int g = 0; g < P::G; ++g)
+#pragma unroll
+          for (int s = 0; s < P::RL; ++s)
+            cp_async_elem(stg + (g * P::RL + s) * NTHR + tid,
+                          src + (lb + (size_t)((t + g * T) + (NX / P::RL) * s) * S) * 2 + c);
+      }
     }
   };
-  if ((int)blockIdx.x < ngroups) issue_loads(blockIdx.x);
+  // register n of this thread out of the staged group
+  auto staged = [&](int n) {
+    if (BULK) {
+      const elem* row = stg + (size_t)line * NX * 2;
+      if (MODE == MODE_PRO || MODE == MODE_FWD) return St::cv(row[(t + ((n + 8 * c) & 15) * T) * 2 + c]);
+      const int g = n / P::RL, s = n % P::RL;
+      return St::cv(row[((t + g * T) + (NX / P::RL) * s) * 2 + c]);
+    } else {
+      return St::cv(stg[n * NTHR + tid]);
+    }
+  };
+  if (tid == 0) {
+    mbar_init(&full, 1);
+    mbar_init(&ffull, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  // Work distribution: the group of iteration it+1 is in `nxt` (thread 0), fetched with the atomic one iteration
+  // ahead so that its latency never sits in front of a barrier; published to the CTA through next_s.  As soon as it is
+  // known, the group's psi rows and field rows are requested into L2, a whole period before they are copied.
+  int nxt = ngroups;
+  __syncthreads();  // the barriers are initialised before anyone waits on them
+  pdl_wait();  // psi and the work counter belong to the preceding kernel
+  if ((int)blockIdx.x < ngroups) {
+    issue_loads(blockIdx.x);
+    if (tid == 0) nxt = sched_next(a.sched);
+  }
+  auto prefetch_group_l2 = [&](int grp) {  // thread 0
+    if (S != 1 || grp >= ngroups || !(a.dbg & 4)) return;
+    const size_t first = (size_t)grp * LINES * NX;
+    prefetch_l2_bulk(reinterpret_cast<const elem*>(a.src) + first * 2, GROUP_BYTES);
+    if (MODE != MODE_FWD) {
+      constexpr unsigned FB = LINES * NX * (unsigned)sizeof(real);
+      if (a.V) prefetch_l2_bulk(reinterpret_cast<const real*>(a.V) + first, FB);
+      if (a.Om) prefetch_l2_bulk(reinterpret_cast<const real*>(a.Om) + first, FB);
+      if (a.De) prefetch_l2_bulk(reinterpret_cast<const real*>(a.De) + first, FB);
+    }
+  };
 
   __shared__ double red[2][32];
   __shared__ int next_s[2];  // group this CTA takes next (written by thread 0, double-buffered over iterations)
@@ -254,12 +327,14 @@ pass_x_kernel(const PassXArgs a) {
   for (int grp = blockIdx.x; grp < ngroups; ++it) {
     const size_t first_point = (size_t)grp * LINES * NX;  // first point of the CTA's lines (xs = 1)
     const size_t lbase = line_base(grp * LINES + line);
-    // the next group is requested now and published before the last barrier of this iteration (latency hidden)
-    int nxt_req = 0;
-    if (tid == 0) nxt_req = sched_next(a.sched);
-    cp_async_wait_all();
+    if (tid == 0) {
+      next_s[it & 1] = nxt;  // visible to the CTA behind the next barrier
+      prefetch_group_l2(nxt);
+    }
+    cp_async_wait_all();  // twiddle table (first iteration), staged rows of a split axis
+    if (BULK) mbar_wait(&full, it & 1);
 #pragma unroll
-    for (int n = 0; n < 16; ++n) v[n] = St::cv(stg[n * NTHR + tid]);
+    for (int n = 0; n < 16; ++n) v[n] = staged(n);
     if (MODE == MODE_PRO && a.scale != nullptr) {
       const double s = a.scale[c];
 #pragma unroll
@@ -272,7 +347,7 @@ pass_x_kernel(const PassXArgs a) {
     // radix-16 stage), so it runs under that stage's twiddles and butterflies.
     auto fields_hook = [&]() {
       __syncthreads();
-      stage_fields<DT, NX, LINES, XS>(smem, a, first_point, grp * LINES, tid);
+      stage_fields<DT, NX, LINES, XS>(smem, a, first_point, grp * LINES, tid, &ffull, FBULK);
     };
     if (MODE == MODE_MID || MODE == MODE_EPI) line_fft_inv<NX>(buf, twS, t, c, v, flip, fields_hook);
     TL_MARK(1);
@@ -280,11 +355,13 @@ pass_x_kernel(const PassXArgs a) {
     if (MODE != MODE_FWD) {
       if (MODE == MODE_PRO) fields_hook();
       cp_async_wait_all();
-      __syncthreads();
+      if (FBULK) mbar_wait(&ffull, it & 1);
+      // zero fills and cp.async copies are per-thread writes: a barrier makes them visible; bulk copies
+      // complete on the mbarrier every thread has just waited on
+      if (!FBULK || a.V == nullptr || a.Om == nullptr || a.De == nullptr) __syncthreads();
       TL_MARK(2);
       real_space<DT, NX, LINES, MODE>(v, a, smem, line, t, c, lc, sm, so);
       TL_MARK(3);
-      if (MODE == MODE_EPI && tid == 0) next_s[it & 1] = nxt_req;
       if (MODE == MODE_EPI && a.want_norm) {
         // norm partials of this row group, one slot per group: the sums do not depend on which CTA took the group,
         // so the reduction order (and every imaginary-time result) is the same from run to run.  Each lane summed
@@ -308,19 +385,20 @@ pass_x_kernel(const PassXArgs a) {
       }
     }
 
-    int nxt_grp;
+    if (MODE != MODE_EPI) {
+      fwd_stages<NX, 1>(buf, twS, t, c, v, flip, CtaSync());
+      __syncthreads();  // the last exchange has been read by every warp: the line buffers are free
+    }
+    const int nxt_grp = next_s[it & 1];
+    TL_MARK(4);
+    if (nxt_grp < ngroups) {  // the line buffers are free: the next group may land
+      issue_loads(nxt_grp);
+      if (tid == 0) nxt = sched_next(a.sched);  // consumed in the next iteration
+    }
     if (MODE == MODE_EPI) {
-      nxt_grp = next_s[it & 1];
-      if (nxt_grp < ngroups) issue_loads(nxt_grp);  // the line buffers are free after the real-space part
 #pragma unroll
       for (int n = 0; n < 16; ++n) St::st(a.dst, (lbase + (size_t)(t + ((n + 8 * c) & 15) * T) * S) * 2 + c, v[n]);
     } else {
-      fwd_stages<NX, 1>(buf, twS, t, c, v, flip, CtaSync());
-      if (tid == 0) next_s[it & 1] = nxt_req;
-      __syncthreads();  // the last exchange has been read by every warp: the line buffers are free
-      nxt_grp = next_s[it & 1];
-      TL_MARK(4);
-      if (nxt_grp < ngroups) issue_loads(nxt_grp);
       dft_last<-1, P::RL>(v);
       TL_MARK(5);
       // the k_x phase of the k-space factor is applied by the column pass (one table value per thread there)
@@ -331,12 +409,6 @@ pass_x_kernel(const PassXArgs a) {
           const int off = g * T + (NX / P::RL) * s;
           St::st(a.dst, (lbase + (size_t)(t + off) * S) * 2 + c, v[g * P::RL + s]);
         }
-    }
-    if (MODE != MODE_FWD && S == 1 && tid == 0 && nxt_grp < ngroups) {  // field rows of the next group: into L2
-      const size_t nxt = (size_t)nxt_grp * LINES * NX;
-      if (a.V) prefetch_l2_bulk(reinterpret_cast<const real*>(a.V) + nxt, LINES * NX * (unsigned)sizeof(real));
-      if (a.Om) prefetch_l2_bulk(reinterpret_cast<const real*>(a.Om) + nxt, LINES * NX * (unsigned)sizeof(real));
-      if (a.De) prefetch_l2_bulk(reinterpret_cast<const real*>(a.De) + nxt, LINES * NX * (unsigned)sizeof(real));
     }
     TL_MARK(6);
     TL_TILE();

@@ -38,6 +38,8 @@ int plan_lines_x(int n) {
 }
 int plan_lines_ydb(int n) { return n == 2048 ? Lines<2048>::YDB : (n == 1024 ? Lines<1024>::YDB : 0); }
 
+bool plan_has_duo(int n) { return n == 2048 ? Lines<2048>::DUO : (n == 1024 ? Lines<1024>::DUO : false); }
+
 int plan_tw_total(int n) {
   PlanInfo p = plan_info(n);
   int total = 0;
