@@ -40,7 +40,7 @@ struct PassXArgs {
   double cell;           // dx dy
   int norm_mode;         // SPGPE_NORM_PER_COMPONENT | SPGPE_NORM_TOTAL
   const double* fmax;    // [3] device: max |V|, max |Omega|, max |delta| over the grid (tier bounds)
-  int dbg;               // experiment switches (bit 0: psi rows by bulk copy, 1: field rows by bulk copy, 2: early L2 prefetch)
+  int dbg;               // experiment switches (bit 0: psi rows by bulk copy, 1: field rows by per-thread cp.async instead of bulk copies, 2: early L2 prefetch)
 };
 
 __device__ __forceinline__ double shfl_xor_d(double x, int m) { return __shfl_xor_sync(0xffffffffu, x, m); }
@@ -253,7 +253,7 @@ pass_x_kernel(const PassXArgs a) {
   elem* stg = reinterpret_cast<elem*>(smem);
   constexpr int S = XS;  // == a.xs
   const bool BULK = (XS == 1) && (a.dbg & 1);
-  const bool FBULK = (XS == 1) && (a.dbg & 2);
+  const bool FBULK = (XS == 1) && !(a.dbg & 2);
   constexpr unsigned GROUP_BYTES = (unsigned)LINES * NX * 2 * (unsigned)sizeof(elem);
   __shared__ __align__(8) unsigned long long full, ffull;  // psi rows landed / field rows landed
   // point index of position 0 of line L: lines are rows (xs = 1) or the even / odd points of a row (xs = 2)

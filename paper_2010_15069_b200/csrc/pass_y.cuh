@@ -318,7 +318,10 @@ __global__ void __launch_bounds__(LINES * (NY / 8), 1) pass_y_db_kernel(const __
   for (int g = 0; g < P::G; ++g)
 #pragma unroll
     for (int s = 0; s < P::RL; ++s) eyr[g * P::RL + s] = __ldg(a.eyk + (t + g * T) + (NY / P::RL) * s);
-  if (tid == 0) {
+  // the loading thread initialises the barriers itself: its first expect_tx follows the initialisation in program
+  // order (initialised by another warp, the first load could reach an uninitialised barrier and the tile would never
+  // be seen as landed); every other thread meets the barriers behind the __syncthreads below
+  if (tid == LT) {
     mbar_init(&mbar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
