@@ -27,7 +27,7 @@ class OrcParams(ctypes.Structure):
         ("Lx", ctypes.c_double), ("Ly", ctypes.c_double),
         ("g_uu", ctypes.c_double), ("g_dd", ctypes.c_double), ("g_ud", ctypes.c_double),
         ("k_L", ctypes.c_double),
-        ("norm_mode", ctypes.c_int), ("naive_max", ctypes.c_int),
+        ("norm_mode", ctypes.c_int), ("naive_max", ctypes.c_int), ("rs_split", ctypes.c_int),
     ]
 
 
@@ -63,14 +63,15 @@ def _psi_ptr(psi: np.ndarray):
     return psi.ctypes.data_as(ctypes.c_void_p)
 
 
-def params(nx, ny, Lx, Ly, g_uu=0.0, g_dd=0.0, g_ud=0.0, k_L=0.0, norm_mode=0, naive_max=32) -> OrcParams:
+def params(nx, ny, Lx, Ly, g_uu=0.0, g_dd=0.0, g_ud=0.0, k_L=0.0, norm_mode=0, naive_max=32,
+           rs_split=0) -> OrcParams:
     return OrcParams(int(nx), int(ny), float(Lx), float(Ly), float(g_uu), float(g_dd), float(g_ud),
-                     float(k_L), int(norm_mode), int(naive_max))
+                     float(k_L), int(norm_mode), int(naive_max), int(rs_split))
 
 
-def params_of(w, naive_max=32) -> OrcParams:
+def params_of(w, naive_max=32, rs_split=0) -> OrcParams:
     """OrcParams of a workloads.Workload."""
-    return params(w.nx, w.ny, w.Lx, w.Ly, w.g_uu, w.g_dd, w.g_ud, w.k_L, w.norm_mode, naive_max)
+    return params(w.nx, w.ny, w.Lx, w.Ly, w.g_uu, w.g_dd, w.g_ud, w.k_L, w.norm_mode, naive_max, rs_split)
 
 
 def set_threads(n: int) -> None:
@@ -161,3 +162,56 @@ def energy(psi, V, Om, de, p: OrcParams) -> np.ndarray:
     out = np.empty(5)
     lib().orc_energy(_psi_ptr(psi), _dp(V), _dp(Om), _dp(de), ctypes.byref(p), _dp(out))
     return out
+
+
+def half_nested(psi, V, Om, de, p: OrcParams, tau: float, imag: int) -> np.ndarray:
+    """D(tau/2) X(tau) D(tau/2) whatever p.rs_split says."""
+    out = np.array(psi, dtype=np.complex128, order="C", copy=True)
+    lib().orc_half_nested(_psi_ptr(out), _dp(V), _dp(Om), _dp(de), ctypes.byref(p), ctypes.c_double(tau), int(imag))
+    return out
+
+
+def anneal_noise(psi, p: OrcParams, seed: int, event: int, amp: float) -> np.ndarray:
+    """psi + the Gaussian noise of annealing event `event` (counter-based generator of the C file)."""
+    out = np.array(psi, dtype=np.complex128, order="C", copy=True)
+    lib().orc_anneal_noise(_psi_ptr(out), ctypes.byref(p), ctypes.c_ulonglong(seed & 0xFFFFFFFFFFFFFFFF),
+                           ctypes.c_longlong(event), ctypes.c_double(amp))
+    return out
+
+
+def step_anneal(psi, V, Om, de, p: OrcParams, n: int, dt: float, every: int, amp: float, seed: int,
+                first_step: int = 0, targets: Optional[Sequence[float]] = None) -> np.ndarray:
+    """n imaginary-time steps; noise event j/every enters step j when j > 0 and j % every == 0."""
+    out = np.array(psi, dtype=np.complex128, order="C", copy=True)
+    t = np.array(norm(out, p) if targets is None else targets, dtype=np.float64)
+    lib().orc_step_anneal(_psi_ptr(out), _dp(V), _dp(Om), _dp(de), ctypes.byref(p), int(n), ctypes.c_double(dt),
+                          _dp(t), ctypes.c_longlong(first_step), int(every), ctypes.c_double(amp),
+                          ctypes.c_ulonglong(seed & 0xFFFFFFFFFFFFFFFF))
+    return out
+
+
+def observables(psi, p: OrcParams) -> np.ndarray:
+    """[N_up, N_dn, I_uu, I_dd, I_ud, s] (Eq. 14)."""
+    psi = np.ascontiguousarray(psi, dtype=np.complex128)
+    out = np.empty(6)
+    lib().orc_observables(_psi_ptr(psi), ctypes.byref(p), _dp(out))
+    return out
+
+
+def kspace_observables(hat, p: OrcParams) -> np.ndarray:
+    """[M_up, M_dn, T_up, T_dn, P_up, P_dn] of a forward-transformed order parameter."""
+    hat = np.ascontiguousarray(hat, dtype=np.complex128)
+    out = np.empty(6)
+    lib().orc_kspace_observables(_psi_ptr(hat), ctypes.byref(p), _dp(out))
+    return out
+
+
+def step_observe(psi, V, Om, de, p: OrcParams, n: int, dt: float, imag: int,
+                 targets: Optional[Sequence[float]] = None):
+    """(psi after n steps, real-space observables of it, k-space observables in the middle of the last step)."""
+    out = np.array(psi, dtype=np.complex128, order="C", copy=True)
+    t = np.array(norm(out, p) if targets is None else targets, dtype=np.float64)
+    o_r, o_k = np.empty(6), np.empty(6)
+    lib().orc_step_observe(_psi_ptr(out), _dp(V), _dp(Om), _dp(de), ctypes.byref(p), int(n), ctypes.c_double(dt),
+                           int(imag), _dp(t), _dp(o_r), _dp(o_k))
+    return out, o_r, o_k

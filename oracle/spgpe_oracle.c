@@ -17,7 +17,11 @@
  * check that does not come from this file: naive-DFT and numpy.fft equality, exact
  * plane-wave solution, Rabi closed form, scipy.linalg.expm for the SU(2) factor,
  * Eq. 11 band minima, Gaussian ground-state energy, decay rate e^{-tau} of the first
- * excited state, norm / energy conservation, reversibility, order of convergence.
+ * excited state, norm / energy conservation, reversibility, order of convergence;
+ * the operator order of orc_step against a numpy.fft / scipy expm composition; the nested
+ * split against per-point expm factors and its order 2 of convergence; the annealing noise
+ * against an independent numpy evaluation of the same counter stream and its moments; the
+ * observables against closed forms on uniform / separated states and numpy sums.
  * Nothing here is "parity unpinned".
  *
  * Layout (same as the C ABI of include/spgpe.h): psi[iy][ix][c] complex128, c = 0 (up),
@@ -38,6 +42,8 @@ typedef struct {
     double k_L;              /* signed recoil wavenumber, Eq. 5, R-2 */
     int norm_mode;           /* 0: per component (BASELINE.json), 1: total, R-7 */
     int naive_max;           /* per-axis length up to which the O(N^2) DFT is used (default 32) */
+    int rs_split;            /* real-space part: 0 = one 2x2 exponential (north_star, R-5),
+                                1 = nested second-order split D(tau/2) X(tau) D(tau/2) (R-15) */
 } orc_params;
 
 static const double ORC_PI = 3.14159265358979323846264338327950288;
@@ -232,9 +238,15 @@ void orc_su2(double a, double bx, double bz, double tau, int imag, double *U) {
  * Densities are those of the psi that ENTERS the call (R-6).
  * d_up = V + g_uu n_up + g_ud n_dn + delta/2;  d_dn = V + g_dd n_dn + g_ud n_up - delta/2
  * a = (d_up + d_dn)/2, b_z = (d_up - d_dn)/2, b_x = Omega/2. */
+void orc_half_nested(double *psi, const double *V, const double *Om, const double *de, const orc_params *p,
+                     double tau, int imag);
 void orc_half(double *psi, const double *V, const double *Om, const double *de, const orc_params *p,
               double tau, int imag) {
     const size_t P = (size_t)p->nx * p->ny;
+    if (p->rs_split == 1) {
+        orc_half_nested(psi, V, Om, de, p, tau, imag);
+        return;
+    }
 #pragma omp parallel for schedule(static)
     for (size_t i = 0; i < P; ++i) {
         double ur = psi[4 * i], ui = psi[4 * i + 1], dr = psi[4 * i + 2], di = psi[4 * i + 3];
@@ -249,6 +261,54 @@ void orc_half(double *psi, const double *V, const double *Om, const double *de, 
         psi[4 * i + 1] = U[0] * ui + U[1] * ur + U[2] * di + U[3] * dr;
         psi[4 * i + 2] = U[4] * ur - U[5] * ui + U[6] * dr - U[7] * di;
         psi[4 * i + 3] = U[4] * ui + U[5] * ur + U[6] * di + U[7] * dr;
+    }
+}
+
+/* ---- nested second-order real-space split (the real-space operators U^(2,3,4)
+ * "do not necessarily commute and should be split to second-order"; reading R-15 of DESIGN.md):
+ *   R_nested(tau) = D(tau/2) X(tau) D(tau/2)
+ * D(s): the diagonal factors U^(2) U^(3) and the detuning: psi_c <- e^{-i s d_c} psi_c with
+ *       d_up = V + g_uu n_up + g_ud n_dn + delta/2, d_dn = V + g_dd n_dn + g_ud n_up - delta/2 (Eqs. 6-7),
+ *       densities of the psi that enters D (a diagonal phase does not change them); imaginary time e^{-s d_c}.
+ * X(s): the Raman factor U^(4) = exp(-i s (Omega/2) sigma_x) (Eq. 8): with th = s Omega/2,
+ *       psi_up <- cos(th) psi_up - i sin(th) psi_dn, psi_dn <- -i sin(th) psi_up + cos(th) psi_dn;
+ *       imaginary time: cosh(th), -sinh(th).
+ * The second D uses the densities after X (refreshed), which is what makes the product symmetric. */
+static void nested_diag(double *q, double v, double dl, const orc_params *p, double s, int imag) {
+    double n_up = q[0] * q[0] + q[1] * q[1], n_dn = q[2] * q[2] + q[3] * q[3];
+    double d_up = v + p->g_uu * n_up + p->g_ud * n_dn + 0.5 * dl;
+    double d_dn = v + p->g_dd * n_dn + p->g_ud * n_up - 0.5 * dl;
+    if (!imag) {
+        double cu = cos(d_up * s), su = -sin(d_up * s), cd = cos(d_dn * s), sd = -sin(d_dn * s);
+        double ur = q[0], ui = q[1], dr = q[2], di = q[3];
+        q[0] = ur * cu - ui * su; q[1] = ur * su + ui * cu;
+        q[2] = dr * cd - di * sd; q[3] = dr * sd + di * cd;
+    } else {
+        double eu = exp(-d_up * s), ed = exp(-d_dn * s);
+        q[0] *= eu; q[1] *= eu; q[2] *= ed; q[3] *= ed;
+    }
+}
+void orc_half_nested(double *psi, const double *V, const double *Om, const double *de, const orc_params *p,
+                     double tau, int imag) {
+    const size_t P = (size_t)p->nx * p->ny;
+#pragma omp parallel for schedule(static)
+    for (size_t i = 0; i < P; ++i) {
+        double *q = psi + 4 * i;
+        double v = V ? V[i] : 0.0, om = Om ? Om[i] : 0.0, dl = de ? de[i] : 0.0;
+        nested_diag(q, v, dl, p, 0.5 * tau, imag);
+        double th = 0.5 * om * tau;
+        double ur = q[0], ui = q[1], dr = q[2], di = q[3];
+        if (!imag) {
+            double c = cos(th), s = sin(th);
+            /* -i s (a + i b) = s b - i s a */
+            q[0] = c * ur + s * di; q[1] = c * ui - s * dr;
+            q[2] = c * dr + s * ui; q[3] = c * di - s * ur;
+        } else {
+            double c = cosh(th), s = sinh(th);
+            q[0] = c * ur - s * dr; q[1] = c * ui - s * di;
+            q[2] = c * dr - s * ur; q[3] = c * di - s * ui;
+        }
+        nested_diag(q, v, dl, p, 0.5 * tau, imag);
     }
 }
 
@@ -319,30 +379,32 @@ void orc_norm(const double *psi, const orc_params *p, double *out) {
 
 /* ---- n Strang steps (operator order R-4; P:L138 for the renormalisation):
  * half(dt/2) -> kinetic(dt) -> half(dt/2) -> if imag: norms and rescale to targets (R-7). */
+/* a6 (R-7): rescale to the target norms, per component or in total */
+static void renormalise(double *psi, const orc_params *p, const double *targets) {
+    const size_t P = (size_t)p->nx * p->ny;
+    double nn[2], su, sd;
+    orc_norm(psi, p, nn);
+    if (p->norm_mode == 0) {
+        su = sqrt(targets[0] / nn[0]);
+        sd = sqrt(targets[1] / nn[1]);
+    } else {
+        su = sd = sqrt((targets[0] + targets[1]) / (nn[0] + nn[1]));
+    }
+#pragma omp parallel for schedule(static)
+    for (size_t i = 0; i < P; ++i) {
+        psi[4 * i] *= su;
+        psi[4 * i + 1] *= su;
+        psi[4 * i + 2] *= sd;
+        psi[4 * i + 3] *= sd;
+    }
+}
 void orc_step(double *psi, const double *V, const double *Om, const double *de, const orc_params *p,
               int n, double dt, int imag, const double *targets) {
-    const size_t P = (size_t)p->nx * p->ny;
     for (int s = 0; s < n; ++s) {
         orc_half(psi, V, Om, de, p, 0.5 * dt, imag);
         orc_kinetic(psi, p, dt, imag);
         orc_half(psi, V, Om, de, p, 0.5 * dt, imag);
-        if (imag) {
-            double nn[2], su, sd;
-            orc_norm(psi, p, nn);
-            if (p->norm_mode == 0) {
-                su = sqrt(targets[0] / nn[0]);
-                sd = sqrt(targets[1] / nn[1]);
-            } else {
-                su = sd = sqrt((targets[0] + targets[1]) / (nn[0] + nn[1]));
-            }
-#pragma omp parallel for schedule(static)
-            for (size_t i = 0; i < P; ++i) {
-                psi[4 * i] *= su;
-                psi[4 * i + 1] *= su;
-                psi[4 * i + 2] *= sd;
-                psi[4 * i + 3] *= sd;
-            }
-        }
+        if (imag) renormalise(psi, p, targets);
     }
 }
 
@@ -391,4 +453,117 @@ void orc_energy(const double *psi, const double *V, const double *Om, const doub
     out[3] = w * ei;
     out[4] = w * er;
     out[0] = out[1] + out[2] + out[3] + out[4];
+}
+
+/* ---- annealing noise ("we periodically 'annealed' the system with Gaussian noise to
+ * more quickly find the ground state"; the paper gives neither amplitude nor period: reading R-16 of DESIGN.md).
+ * Counter-based generator (its own implementation here; the CUDA path implements the same definition):
+ *   U(j)  = (mix64(seed + (j+1) * 0x9E3779B97F4A7C15) >> 11) * 2^-53      (splitmix64 output j, 53-bit uniform in [0,1))
+ *   mix64(z): z ^= z >> 30; z *= 0xBF58476D1CE4E5B9; z ^= z >> 27; z *= 0x94D049BB133111EB; z ^= z >> 31
+ * Element e = (iy*nx + ix)*2 + c of annealing event k >= 1 uses the counter q = k * (2 nx ny) + e and the pair
+ * u1 = U(2q), u2 = U(2q+1):  r = sqrt(-2 ln(1 - u1)),  xi = r (cos 2 pi u2 + i sin 2 pi u2)   (Box-Muller),
+ *   psi_e <- psi_e + (amp / sqrt 2) xi        (re and im each N(0, amp^2 / 2), so <|noise|^2> = amp^2). */
+static unsigned long long orc_mix64(unsigned long long z) {
+    z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ULL;
+    z ^= z >> 27; z *= 0x94D049BB133111EBULL;
+    z ^= z >> 31;
+    return z;
+}
+static double orc_uniform(unsigned long long seed, unsigned long long j) {
+    unsigned long long z = orc_mix64(seed + (j + 1ULL) * 0x9E3779B97F4A7C15ULL);
+    return (double)(z >> 11) * (1.0 / 9007199254740992.0);
+}
+void orc_anneal_noise(double *psi, const orc_params *p, unsigned long long seed, long long event, double amp) {
+    const size_t E = (size_t)p->nx * p->ny * 2;
+    const double a = amp / sqrt(2.0);
+#pragma omp parallel for schedule(static)
+    for (size_t e = 0; e < E; ++e) {
+        unsigned long long q = (unsigned long long)event * (unsigned long long)E + (unsigned long long)e;
+        double u1 = orc_uniform(seed, 2ULL * q), u2 = orc_uniform(seed, 2ULL * q + 1ULL);
+        double r = sqrt(-2.0 * log1p(-u1));
+        double ang = 2.0 * ORC_PI * u2;
+        psi[2 * e] += a * r * cos(ang);
+        psi[2 * e + 1] += a * r * sin(ang);
+    }
+}
+
+/* n imaginary-time steps with annealing: j = first_step + s is the index of the step since the schedule began;
+ * when every > 0, j > 0 and j % every == 0 the noise of event j / every is added to the order parameter that enters
+ * step j (the renormalisation at the end of that step restores the norms). */
+void orc_step_anneal(double *psi, const double *V, const double *Om, const double *de, const orc_params *p,
+                     int n, double dt, const double *targets, long long first_step, int every, double amp,
+                     unsigned long long seed) {
+    for (int s = 0; s < n; ++s) {
+        long long j = first_step + s;
+        if (every > 0 && j > 0 && j % every == 0) orc_anneal_noise(psi, p, seed, j / every, amp);
+        orc_step(psi, V, Om, de, p, 1, dt, 1, targets);
+    }
+}
+
+/* ---- observables.
+ * Real space (out_r[6]): N_up, N_dn (R-8), I_uu = dx dy sum rho_up^2, I_dd = dx dy sum rho_dn^2,
+ * I_ud = dx dy sum rho_up rho_dn, and the phase-separation parameter of Eq. 14 (the printed equation carries
+ * both a sum over r and system averages: reading R-17, the system-averaged form)
+ *   s = 1 - <rho_up rho_dn> / sqrt(<rho_up^2> <rho_dn^2>) = 1 - I_ud / sqrt(I_uu I_dd),  rho_c = |psi_c|^2.
+ * k space (out_k[6]) of a TRANSFORMED order parameter hat = F psi (unnormalised forward DFT), per component c:
+ *   M_c = (dx dy/(nx ny)) sum_k |hat_c|^2 (= N_c, Parseval), T_c = (dx dy/(nx ny)) sum_k K_c(k) |hat_c|^2 (kinetic
+ *   energy, R-8), P_c = (dx dy/(nx ny)) sum_k k_x |hat_c|^2 (x momentum); order: M_up, M_dn, T_up, T_dn, P_up, P_dn. */
+void orc_observables(const double *psi, const orc_params *p, double *out_r) {
+    const size_t P = (size_t)p->nx * p->ny;
+    const double w = (p->Lx / p->nx) * (p->Ly / p->ny);
+    double nu = 0.0, nd = 0.0, uu = 0.0, dd = 0.0, ud = 0.0;
+#pragma omp parallel for reduction(+ : nu, nd, uu, dd, ud) schedule(static)
+    for (size_t i = 0; i < P; ++i) {
+        double ru = psi[4 * i] * psi[4 * i] + psi[4 * i + 1] * psi[4 * i + 1];
+        double rd = psi[4 * i + 2] * psi[4 * i + 2] + psi[4 * i + 3] * psi[4 * i + 3];
+        nu += ru; nd += rd; uu += ru * ru; dd += rd * rd; ud += ru * rd;
+    }
+    out_r[0] = w * nu; out_r[1] = w * nd; out_r[2] = w * uu; out_r[3] = w * dd; out_r[4] = w * ud;
+    out_r[5] = 1.0 - ud / sqrt(uu * dd);
+}
+void orc_kspace_observables(const double *hat, const orc_params *p, double *out_k) {
+    const int nx = p->nx, ny = p->ny;
+    const double w = (p->Lx / nx) * (p->Ly / ny) / ((double)nx * (double)ny);
+    double *Kxu = (double *)malloc(sizeof(double) * (size_t)nx);
+    double *Kxd = (double *)malloc(sizeof(double) * (size_t)nx);
+    double *Ky = (double *)malloc(sizeof(double) * (size_t)ny);
+    double *kx = (double *)malloc(sizeof(double) * (size_t)nx);
+    orc_kinetic_tables(p, Kxu, Kxd, Ky);
+    orc_kgrid(nx, p->Lx, kx);
+    double mu = 0.0, md = 0.0, tu = 0.0, td = 0.0, pu = 0.0, pd = 0.0;
+#pragma omp parallel for reduction(+ : mu, md, tu, td, pu, pd) schedule(static)
+    for (int iy = 0; iy < ny; ++iy) {
+        for (int ix = 0; ix < nx; ++ix) {
+            size_t i = (size_t)iy * nx + ix;
+            double ru = hat[4 * i] * hat[4 * i] + hat[4 * i + 1] * hat[4 * i + 1];
+            double rd = hat[4 * i + 2] * hat[4 * i + 2] + hat[4 * i + 3] * hat[4 * i + 3];
+            mu += ru; md += rd;
+            tu += (Kxu[ix] + Ky[iy]) * ru; td += (Kxd[ix] + Ky[iy]) * rd;
+            pu += kx[ix] * ru; pd += kx[ix] * rd;
+        }
+    }
+    free(Kxu); free(Kxd); free(Ky); free(kx);
+    out_k[0] = w * mu; out_k[1] = w * md; out_k[2] = w * tu; out_k[3] = w * td; out_k[4] = w * pu; out_k[5] = w * pd;
+}
+
+/* n Strang steps with the observables of the fused call spgpe_step_observe (include/spgpe.h): the k-space sums are
+ * those of the order parameter in the middle of the LAST step (after its first half-step and the forward transform;
+ * the k-space phase has unit modulus in real time, so before or after it is the same; in imaginary time: before it),
+ * the real-space ones those of the final state (after the renormalisation in imaginary time). */
+void orc_step_observe(double *psi, const double *V, const double *Om, const double *de, const orc_params *p,
+                      int n, double dt, int imag, const double *targets, double *out_r, double *out_k) {
+    const size_t P = (size_t)p->nx * p->ny;
+    if (n > 1) orc_step(psi, V, Om, de, p, n - 1, dt, imag, targets);
+    if (n >= 1) {
+        double *hat = (double *)malloc(sizeof(double) * 4 * P);
+        orc_half(psi, V, Om, de, p, 0.5 * dt, imag);
+        memcpy(hat, psi, sizeof(double) * 4 * P);
+        orc_fft2(hat, p, -1);
+        orc_kspace_observables(hat, p, out_k);
+        free(hat);
+        orc_kinetic(psi, p, dt, imag);
+        orc_half(psi, V, Om, de, p, 0.5 * dt, imag);
+        if (imag) renormalise(psi, p, targets);
+    }
+    orc_observables(psi, p, out_r);
 }
