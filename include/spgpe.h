@@ -43,6 +43,7 @@ typedef struct spgpe_ctx* spgpe_handle; /* opaque */
 
 enum { SPGPE_C128 = 0, SPGPE_C64 = 1 }; /* storage precision of psi and fields (arithmetic is fp64) */
 enum { SPGPE_NORM_PER_COMPONENT = 0, SPGPE_NORM_TOTAL = 1 }; /* R-7 */
+enum { SPGPE_RS_EXPONENTIAL = 0, SPGPE_RS_NESTED = 1 };      /* form of the real-space part R(tau), R-5 / R-15 */
 
 enum {
   SPGPE_OK = 0,
@@ -91,6 +92,40 @@ int spgpe_set_norm_targets(spgpe_handle h, double n_up, double n_dn);
  * time, return SPGPE_ERR_INVALID_ARG.  A component whose norm is zero keeps scale 1 (it stays zero).  Asynchronous.
  * step(n) then step(m) equals step(n+m) to rounding. */
 int spgpe_step(spgpe_handle h, int n, double dt, int imag);
+
+/* Form of the real-space part R(tau) used by later steps (host-side switch, no device work):
+ *   SPGPE_RS_EXPONENTIAL (default): one 2x2 exponential of the whole local matrix, densities frozen at entry (R-5);
+ *     second order in dt when Omega = 0 or all g are equal, first order otherwise.
+ *   SPGPE_RS_NESTED: the paper's remark that the real-space operators "do not necessarily commute and should be split
+ *     to second-order", read as (R-15)  R(tau) = D(tau/2) X(tau) D(tau/2),  D(s) = exp(-i s diag(d_up, d_dn)),
+ *     d_up = V + g_uu n_up + g_ud n_dn + delta/2, d_dn = V + g_dd n_dn + g_ud n_up - delta/2 with the densities of the
+ *     psi entering D, X(s) = exp(-i s (Omega/2) sigma_x); imaginary time with the decaying counterparts.  Second order
+ *     for every parameter set and exactly reversible in real time.  No extra memory traffic. */
+int spgpe_set_real_space_split(spgpe_handle h, int mode);
+
+/* Annealing of imaginary-time runs ("we periodically 'annealed' the system with Gaussian noise"; the paper
+ * states neither period nor amplitude: R-16).  Counting the imaginary-time steps taken since this call as j = 0, 1, ...,
+ * the order parameter that enters step j receives complex Gaussian noise when every > 0, j > 0 and j % every == 0
+ * (event k = j / every); the renormalisation at the end of that step restores the norms.  every = 0 switches it off.
+ * The noise is a counter-based stream, the same for any launch geometry: element e = (iy*nx + ix)*2 + c of event k uses
+ * q = k * (2 nx ny) + e and the uniforms U(2q), U(2q+1),
+ *   U(j) = (mix64(seed + (j+1) * 0x9E3779B97F4A7C15) >> 11) * 2^-53          (output j of splitmix64),
+ *   mix64(z): z ^= z >> 30; z *= 0xBF58476D1CE4E5B9; z ^= z >> 27; z *= 0x94D049BB133111EB; z ^= z >> 31,
+ *   psi_e += (amp / sqrt 2) sqrt(-2 ln(1 - U(2q))) exp(2 pi i U(2q+1))       (<|noise|^2> = amp^2),
+ * generated in fp64 inside the row pass (no extra sweep over psi).  amp >= 0. */
+int spgpe_set_annealing(spgpe_handle h, int every, double amp, unsigned long long seed);
+
+/* spgpe_step(n, dt, imag), n >= 1, with the observables accumulated inside the passes of the LAST step (no extra
+ * sweep over psi); synchronises.  h_out (host, 12 doubles):
+ *   [0..5]  of the final state: N_up, N_dn, I_uu = dx dy sum rho_up^2, I_dd, I_ud = dx dy sum rho_up rho_dn and the
+ *           phase-separation parameter of Eq. 14 (system-averaged reading R-17)
+ *           s = 1 - <rho_up rho_dn> / sqrt(<rho_up^2> <rho_dn^2>) = 1 - I_ud / sqrt(I_uu I_dd),  rho_c = |psi_c|^2;
+ *   [6..11] of the order parameter in the middle of the last step (after its first half-step, in front of the k-space
+ *           factor), from its transform psi^: M_c = (dx dy / nx ny) sum_k |psi^_c|^2 (= its N_c), kinetic energy
+ *           T_c = (dx dy / nx ny) sum_k K_c |psi^_c|^2 (R-8) and x momentum P_c = (dx dy / nx ny) sum_k k_x |psi^_c|^2,
+ *           in the order M_up, M_dn, T_up, T_dn, P_up, P_dn.
+ * Grids with an axis longer than 4096 return SPGPE_ERR_UNSUPPORTED. */
+int spgpe_step_observe(spgpe_handle h, int n, double dt, int imag, double h_out[12]);
 
 /* N_c = dx dy sum_r |psi_c|^2 (R-8); out = {N_up, N_dn}; synchronises. */
 int spgpe_norm(spgpe_handle h, double out[2]);

@@ -21,6 +21,7 @@ from . import _build
 
 SPGPE_C128, SPGPE_C64 = 0, 1
 SPGPE_NORM_PER_COMPONENT, SPGPE_NORM_TOTAL = 0, 1
+SPGPE_RS_EXPONENTIAL, SPGPE_RS_NESTED = 0, 1
 
 # every symbol include/spgpe.h declares (tests check the library exports exactly these)
 ABI_SYMBOLS = (
@@ -28,7 +29,8 @@ ABI_SYMBOLS = (
     "spgpe_set_potential", "spgpe_set_raman", "spgpe_set_zeeman",
     "spgpe_set_potential_host", "spgpe_set_raman_host", "spgpe_set_zeeman_host",
     "spgpe_set_psi", "spgpe_get_psi", "spgpe_set_psi_host", "spgpe_get_psi_host", "spgpe_set_norm_targets",
-    "spgpe_step", "spgpe_norm", "spgpe_energy", "spgpe_synchronize", "spgpe_launch_count",
+    "spgpe_step", "spgpe_step_observe", "spgpe_set_real_space_split", "spgpe_set_annealing",
+    "spgpe_norm", "spgpe_energy", "spgpe_synchronize", "spgpe_launch_count",
     "spgpe_profile", "spgpe_profile_read",
     "spgpe_strerror", "spgpe_last_cuda_error", "spgpe_probe_dfma", "spgpe_probe_copy",
 )
@@ -71,6 +73,9 @@ def lib() -> ctypes.CDLL:
         L.spgpe_synchronize.argtypes = [vp]
         L.spgpe_set_norm_targets.argtypes = [vp, cd, cd]
         L.spgpe_step.argtypes = [vp, ci, cd, ci]
+        L.spgpe_step_observe.argtypes = [vp, ci, cd, ci, ctypes.POINTER(cd)]
+        L.spgpe_set_real_space_split.argtypes = [vp, ci]
+        L.spgpe_set_annealing.argtypes = [vp, ci, cd, ctypes.c_ulonglong]
         L.spgpe_norm.argtypes = [vp, ctypes.POINTER(cd)]
         L.spgpe_energy.argtypes = [vp, ctypes.POINTER(cd)]
         L.spgpe_launch_count.argtypes = [vp]
@@ -206,6 +211,21 @@ def spgpe_set_norm_targets(h: Handle, n_up: float, n_dn: float) -> None:
 
 def spgpe_step(h: Handle, n: int, dt: float, imag: int = 0) -> None:
     _check(lib().spgpe_step(h.ptr, int(n), float(dt), int(imag)))
+
+
+def spgpe_step_observe(h: Handle, n: int, dt: float, imag: int = 0) -> np.ndarray:
+    """n steps; [N_up, N_dn, I_uu, I_dd, I_ud, s, M_up, M_dn, T_up, T_dn, P_up, P_dn] (include/spgpe.h)."""
+    out = (ctypes.c_double * 12)()
+    _check(lib().spgpe_step_observe(h.ptr, int(n), float(dt), int(imag), out))
+    return np.array(out[:])
+
+
+def spgpe_set_real_space_split(h: Handle, mode: int) -> None:
+    _check(lib().spgpe_set_real_space_split(h.ptr, int(mode)))
+
+
+def spgpe_set_annealing(h: Handle, every: int, amp: float, seed: int) -> None:
+    _check(lib().spgpe_set_annealing(h.ptr, int(every), float(amp), ctypes.c_ulonglong(seed & 0xFFFFFFFFFFFFFFFF)))
 
 
 def spgpe_norm(h: Handle) -> np.ndarray:

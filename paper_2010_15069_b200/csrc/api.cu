@@ -31,6 +31,13 @@ struct spgpe_ctx {
   const void *V, *Om, *De;     // NULL = zero field
   double2 *tw_x, *tw_y;
   double *Kx, *Ky;       // kinetic tables in stored order: Kx[2][nx], Ky[ny]
+  double* kxv;           // k_x in stored order [nx] (observables)
+  double* kpartial;      // [KPARTIAL_ROWS][6] k-space sums of the observed column pass
+  int rs_split;          // SPGPE_RS_EXPONENTIAL | SPGPE_RS_NESTED
+  int anneal_every;      // annealing period in imaginary-time steps (0: off)
+  double anneal_amp;
+  unsigned long long anneal_seed;
+  long long imag_steps;  // imaginary-time steps taken since spgpe_set_annealing
   double2 *exk, *eyk;    // phase tables of (tab_dt, tab_imag)
   double tab_dt;
   int tab_imag;
@@ -77,6 +84,7 @@ static cudaError_t prof_end(spgpe_ctx* h) {
 }
 
 static thread_local char g_cuda_err[256] = "";
+static const int KPARTIAL_ROWS = 4096;  // >= CTAs of any column-pass launch
 
 // Every entry point that takes a handle runs with the handle's device current and restores the caller's device on
 // return (a handle created on GPU 1 keeps working when the caller has switched to GPU 0 in between).
@@ -187,10 +195,12 @@ static cudaError_t dispatch_y(spgpe_ctx* h, int ymode, const PassYArgs& a) {
 }
 
 // kinetic tables in the stored order of the transforms (Eq. 5; R-2, R-3, R-9)
-static void fill_ktables(const spgpe_ctx* h, std::vector<double>& Kx, std::vector<double>& Ky) {
+static void fill_ktables(const spgpe_ctx* h, std::vector<double>& Kx, std::vector<double>& Ky,
+                         std::vector<double>& kxv) {
   const double two_pi = 6.283185307179586476925286766559;
   Kx.resize(2 * (size_t)h->nx);
   Ky.resize(h->ny);
+  kxv.resize(h->nx);
   // unsplit axis: entry pos belongs to the frequency stored at pos; split axis: entry f belongs to frequency f
   for (int pos = 0; pos < h->nx; ++pos) {
     const int f = h->sx == 1 ? plan_freq_of_pos(h->nx, pos) : pos;
@@ -198,6 +208,7 @@ static void fill_ktables(const spgpe_ctx* h, std::vector<double>& Kx, std::vecto
     const double k = two_pi * (double)mt / h->Lx;
     Kx[pos] = 0.5 * (k + h->p.k_L) * (k + h->p.k_L);
     Kx[h->nx + pos] = 0.5 * (k - h->p.k_L) * (k - h->p.k_L);
+    kxv[pos] = k;
   }
   for (int pos = 0; pos < h->ny; ++pos) {
     const int f = h->sy == 1 ? plan_freq_of_pos(h->ny, pos) : pos;
@@ -249,7 +260,7 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
     delete h;
     return SPGPE_ERR_NO_MEMORY;
   }
-  h->partial_cap = 4 * (nx > ny ? nx : ny);  // >= 2 doubles per row group of the row pass (at most 2 ny groups)
+  h->partial_cap = 16 * (nx > ny ? nx : ny);  // up to 8 doubles per row group of the row pass (at most 2 ny groups)
   if (h->partial_cap < 4 * 2048) h->partial_cap = 4 * 2048;
 
   cudaError_t e = cudaSuccess;
@@ -265,12 +276,14 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
   alloc((void**)&h->tw_y, sizeof(double2) * twy);
   alloc((void**)&h->Kx, sizeof(double) * 2 * nx);
   alloc((void**)&h->Ky, sizeof(double) * ny);
+  alloc((void**)&h->kxv, sizeof(double) * nx);
+  alloc((void**)&h->kpartial, sizeof(double) * 6 * KPARTIAL_ROWS);
   alloc((void**)&h->exk, sizeof(double2) * 2 * nx);
   alloc((void**)&h->eyk, sizeof(double2) * ny);
   alloc((void**)&h->partial, sizeof(double) * h->partial_cap);
   alloc((void**)&h->scale, sizeof(double) * 2);
   alloc((void**)&h->target, sizeof(double) * 2);
-  alloc((void**)&h->dout, sizeof(double) * 8);
+  alloc((void**)&h->dout, sizeof(double) * 24);
   alloc((void**)&h->sched, sizeof(int) * 4);
   if (e == cudaSuccess) e = cudaMemset(h->sched, 0, sizeof(int) * 4);
   alloc((void**)&h->fmax, sizeof(double) * 3);
@@ -285,10 +298,11 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
     }
   }
   if (e == cudaSuccess) {
-    std::vector<double> Kx, Ky;
-    fill_ktables(h, Kx, Ky);
+    std::vector<double> Kx, Ky, kxv;
+    fill_ktables(h, Kx, Ky, kxv);
     e = cudaMemcpy(h->Kx, Kx.data(), sizeof(double) * Kx.size(), cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(h->Ky, Ky.data(), sizeof(double) * Ky.size(), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(h->kxv, kxv.data(), sizeof(double) * kxv.size(), cudaMemcpyHostToDevice);
   }
   // join tables of the split axes
   for (int ax = 0; ax < 2 && e == cudaSuccess; ++ax) {
@@ -324,7 +338,7 @@ extern "C" int spgpe_destroy(spgpe_handle h) {
   if (!h) return SPGPE_ERR_INVALID_ARG;
   ON_DEVICE(h);
   cudaStreamSynchronize(h->stream);
-  void* ptrs[] = {h->psi, h->scratch, h->Vbuf, h->Ombuf, h->Debuf, h->tw_x, h->tw_y, h->Kx, h->Ky,
+  void* ptrs[] = {h->psi, h->scratch, h->Vbuf, h->Ombuf, h->Debuf, h->tw_x, h->tw_y, h->Kx, h->Ky, h->kxv, h->kpartial,
                   h->exk, h->eyk, h->partial, h->scale, h->target, h->dout, h->fmax, h->sched, h->wcx, h->wcy, h->fpx, h->fpy};
   for (void* p : ptrs)
     if (p) cudaFree(p);
@@ -447,11 +461,14 @@ static cudaError_t kspace_part(spgpe_ctx* h, const PassYArgs& ya) {
   return dispatch_y(h, YMODE_INVONLY, ya);
 }
 
-extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
+// n Strang steps; obs != NULL: the last step's column pass and closing row pass also leave the sums of
+// spgpe_step_observe, which are finished into h->dout[8..19] (device)
+static int step_impl(spgpe_handle h, int n, double dt, int imag, bool obs) {
   if (!h || n < 0 || !(dt == dt) || isinf(dt)) return SPGPE_ERR_INVALID_ARG;
   imag = imag ? 1 : 0;
   if (imag && !(dt > 0.0)) return SPGPE_ERR_INVALID_ARG;  // imaginary time: dt = d tau > 0 (spgpe.h)
   if (!h->ready) return SPGPE_ERR_NOT_READY;
+  if (obs && (n < 1 || h->sx != 1 || h->sy != 1)) return n < 1 ? SPGPE_ERR_INVALID_ARG : SPGPE_ERR_UNSUPPORTED;
   if (n == 0) return SPGPE_OK;
   ON_DEVICE(h);
   int rc = ensure_tables(h, dt, imag);
@@ -463,27 +480,77 @@ extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) {
   xa.tau = 0.5 * dt; xa.hc = h->hc; xa.imag = imag; xa.want_norm = imag; xa.ny = h->ny * h->sx; xa.xs = h->sx;
   xa.fmax = h->fmax; xa.sched = h->sched; xa.dbg = h->env.xdbg;
   xa.target = h->target; xa.scale_out = h->scale; xa.cell = (h->Lx / h->nx) * (h->Ly / h->ny); xa.norm_mode = h->p.norm_mode;
+  xa.nest = h->rs_split == SPGPE_RS_NESTED; xa.pstride = 2;
+  xa.anneal_seed = h->anneal_seed; xa.anneal_amp = h->anneal_amp; xa.anneal_elems = 2ULL * h->points;
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
   ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx * h->sy;
   // the k_x phase rides on the column pass unless a split axis sends the k-space phases to the join kernel
   ya.exk = (h->sx == 1 && h->sy == 1) ? h->exk : nullptr; ya.sched = h->sched + 2; ya.tmap = h->tmap_psi; ya.tmap_db = h->tmap_psi_db; ya.tmap_duo = h->tmap_psi_duo;
+  // the observed column pass (last step only): k-space sums per CTA into kpartial
+  auto last_kspace = [&]() -> cudaError_t {
+    if (!obs) return kspace_part(h, ya);
+    PassYArgs yo = ya;
+    yo.Kx = h->Kx; yo.Ky = h->Ky; yo.kxv = h->kxv; yo.partial = h->kpartial;
+    return dispatch_y(h, YMODE_STEP_OBS, yo);
+  };
   if (!imag) {
     CK(dispatch_x(h, MODE_PRO, xa));
     for (int s = 1; s <= n; ++s) {
-      CK(kspace_part(h, ya));
+      if (s < n) CK(kspace_part(h, ya));
+      else CK(last_kspace());
+      if (s == n && obs) { xa.want_obs = 1; xa.pstride = 8; }
       CK(dispatch_x(h, s < n ? MODE_MID : MODE_EPI, xa));
     }
   } else {
     for (int s = 0; s < n; ++s) {
+      const long long j = h->imag_steps + s;  // index of this step in the annealing schedule
+      xa.anneal_event = (h->anneal_every > 0 && j > 0 && j % h->anneal_every == 0) ? j / h->anneal_every : 0;
       xa.scale = (s > 0) ? h->scale : nullptr;  // rescale of the previous step, applied at load
       CK(dispatch_x(h, MODE_PRO, xa));
-      CK(kspace_part(h, ya));
+      if (s + 1 < n) CK(kspace_part(h, ya));
+      else CK(last_kspace());
+      if (s + 1 == n && obs) { xa.want_obs = 1; xa.pstride = 8; }
       CK(dispatch_x(h, MODE_EPI, xa));  // also writes the rescale factors (last CTA)
     }
+    h->imag_steps += n;
     h->launches++;
     CK(aux_apply_scale(h->dt, h->psi, h->points, h->scale, h->stream));
   }
+  if (obs) {
+    if (h->ygrid > KPARTIAL_ROWS) return SPGPE_ERR_UNSUPPORTED;
+    h->launches += 2;
+    CK(aux_obs_finish(h->partial, h->ny * h->sx / plan_lines_x(h->mx), 8, xa.cell, imag ? h->scale : nullptr,
+                      h->dout + 8, h->stream));
+    CK(aux_sum_partials(h->kpartial, h->ygrid, 6, xa.cell / ((double)h->nx * (double)h->ny), h->dout + 14, h->stream));
+  }
+  return SPGPE_OK;
+}
+
+extern "C" int spgpe_step(spgpe_handle h, int n, double dt, int imag) { return step_impl(h, n, dt, imag, false); }
+
+extern "C" int spgpe_step_observe(spgpe_handle h, int n, double dt, int imag, double out[12]) {
+  if (!out) return SPGPE_ERR_INVALID_ARG;
+  int rc = step_impl(h, n, dt, imag, true);
+  if (rc) return rc;
+  ON_DEVICE(h);
+  CK(cudaMemcpyAsync(out, h->dout + 8, 12 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CK(cudaStreamSynchronize(h->stream));
+  return SPGPE_OK;
+}
+
+extern "C" int spgpe_set_real_space_split(spgpe_handle h, int mode) {
+  if (!h || (mode != SPGPE_RS_EXPONENTIAL && mode != SPGPE_RS_NESTED)) return SPGPE_ERR_INVALID_ARG;
+  h->rs_split = mode;
+  return SPGPE_OK;
+}
+
+extern "C" int spgpe_set_annealing(spgpe_handle h, int every, double amp, unsigned long long seed) {
+  if (!h || every < 0 || !(amp >= 0.0) || isinf(amp)) return SPGPE_ERR_INVALID_ARG;
+  h->anneal_every = every;
+  h->anneal_amp = amp;
+  h->anneal_seed = seed;
+  h->imag_steps = 0;
   return SPGPE_OK;
 }
 

@@ -72,6 +72,39 @@ cudaError_t aux_sum_partials(const double* partial, int nblk, int ncol, double f
   return cudaGetLastError();
 }
 
+// Real-space observables of spgpe_step_observe from the per-row-group sums of the closing row pass
+// (partial[g][stride]: sum rho_up, rho_dn, rho_up^2, rho_dn^2, rho_up rho_dn; fixed order).  scale != NULL (imaginary
+// time): the sums were taken in front of the rescale psi_c <- s_c psi_c and are carried over to the rescaled state.
+// out = {N_up, N_dn, I_uu, I_dd, I_ud, s}, s = 1 - I_ud / sqrt(I_uu I_dd) (Eq. 14, R-17).
+__global__ void obs_finish_kernel(const double* __restrict__ partial, int ngroups, int stride, double cell,
+                                  const double* __restrict__ scale, double* out) {
+  __shared__ double red[1][32];
+  __shared__ double tot[5];
+  for (int col = 0; col < 5; ++col) {
+    double x[1] = {0.0};
+    for (int b = threadIdx.x; b < ngroups; b += blockDim.x) x[0] += partial[(size_t)b * stride + col];
+    double r[1];
+    block_reduce<1>(x, r, red);
+    if (threadIdx.x == 0) tot[col] = r[0];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    const double su = scale ? scale[0] * scale[0] : 1.0, sd = scale ? scale[1] * scale[1] : 1.0;
+    const double uu = tot[2] * su * su, dd = tot[3] * sd * sd, ud = tot[4] * su * sd;
+    out[0] = cell * tot[0] * su;
+    out[1] = cell * tot[1] * sd;
+    out[2] = cell * uu;
+    out[3] = cell * dd;
+    out[4] = cell * ud;
+    out[5] = 1.0 - ud / sqrt(uu * dd);
+  }
+}
+cudaError_t aux_obs_finish(const double* partial, int ngroups, int stride, double cell, const double* scale,
+                           double* out, cudaStream_t s) {
+  obs_finish_kernel<<<1, 256, 0, s>>>(partial, ngroups, stride, cell, scale, out);
+  return cudaGetLastError();
+}
+
 template <int DT>
 __global__ void apply_scale_kernel(void* psi, size_t points, const double* __restrict__ scale) {
   const double s0 = scale[0], s1 = scale[1];

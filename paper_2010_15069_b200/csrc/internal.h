@@ -54,6 +54,9 @@ cudaError_t aux_phase_tables(const double* Kx, const double* Ky, int nx, int ny,
 cudaError_t aux_sum_partials(const double* partial, int nblk, int ncol, double factor, double* out,
                              cudaStream_t s);
 cudaError_t aux_apply_scale(int dt, void* psi, size_t points, const double* scale, cudaStream_t s);
+// real-space observables from partial[ngroups][stride] (aux.cu, obs_finish_kernel); out[6]
+cudaError_t aux_obs_finish(const double* partial, int ngroups, int stride, double cell, const double* scale,
+                           double* out, cudaStream_t s);
 // partial[nblk][2]: sum |psi_c|^2 ; returns nblk used through *nblk (<= max_blk)
 cudaError_t aux_norm_partials(int dt, const void* psi, size_t points, double* partial, int nblk,
                               cudaStream_t s);

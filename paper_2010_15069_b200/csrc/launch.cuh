@@ -188,6 +188,7 @@ cudaError_t launch_y_step(const PassYArgs& a, cudaStream_t s, const LaunchEnv& e
         case YMODE_STEP: return launch_y_step<0, N_>(a, s, env, g);                            \
         case YMODE_ENERGY: return launch_y<0, N_, YMODE_ENERGY>(a, s, env, g);                        \
         case YMODE_FWDONLY: return launch_y<0, N_, YMODE_FWDONLY>(a, s, env, g);                      \
+        case YMODE_STEP_OBS: return launch_y<0, N_, YMODE_STEP_OBS>(a, s, env, g);                    \
         default: return launch_y<0, N_, YMODE_INVONLY>(a, s, env, g);                                 \
       }                                                                                          \
     }                                                                                            \
@@ -195,6 +196,7 @@ cudaError_t launch_y_step(const PassYArgs& a, cudaStream_t s, const LaunchEnv& e
       case YMODE_STEP: return launch_y_step<1, N_>(a, s, env, g);                              \
       case YMODE_ENERGY: return launch_y<1, N_, YMODE_ENERGY>(a, s, env, g);                          \
       case YMODE_FWDONLY: return launch_y<1, N_, YMODE_FWDONLY>(a, s, env, g);                        \
+      case YMODE_STEP_OBS: return launch_y<1, N_, YMODE_STEP_OBS>(a, s, env, g);                      \
       default: return launch_y<1, N_, YMODE_INVONLY>(a, s, env, g);                                   \
     }                                                                                            \
   }

@@ -27,7 +27,7 @@ struct PassXArgs {
   const void* De;
   const double2* tw;     // twiddles of NX
   const double* scale;   // [2] per-component factor applied at load (MODE_PRO, imaginary time) or NULL
-  double* partial;       // [ny / LINES][2] sum |psi_c|^2 of every row group (MODE_EPI with want_norm)
+  double* partial;       // [ny / LINES][pstride] sums of every row group (MODE_EPI with want_norm or want_obs)
   double tau;            // half-step size dt/2
   HalfCoef hc;
   int imag;
@@ -40,11 +40,46 @@ struct PassXArgs {
   double cell;           // dx dy
   int norm_mode;         // SPGPE_NORM_PER_COMPONENT | SPGPE_NORM_TOTAL
   const double* fmax;    // [3] device: max |V|, max |Omega|, max |delta| over the grid (tier bounds)
+  int nest;              // 1: nested second-order split D(tau/2) X(tau) D(tau/2) of the real-space part (su2.cuh)
+  int want_obs;          // MODE_EPI: five partial sums per row group (norms, rho_up^2, rho_dn^2, rho_up rho_dn)
+  int pstride;           // doubles per row group in `partial`: 2 (norms only) or 8 (want_obs)
+  // annealing (MODE_PRO): noise of event `anneal_event` (0: none) added to the order parameter at load
+  long long anneal_event;
+  unsigned long long anneal_seed;
+  unsigned long long anneal_elems;  // 2 nx ny: elements per event
+  double anneal_amp;
   int dbg;               // experiment switches (bit 0: psi rows by bulk copy, 1: field rows by per-thread cp.async instead of bulk copies, 2: early L2 prefetch)
+};
+
+// observables of the final state (MODE_EPI with want_obs): sums of rho_m^2, rho_o^2, rho_m rho_o over the lane's points
+struct ObsSums {
+  double mm, oo, mo;
 };
 
 __device__ __forceinline__ double shfl_xor_d(double x, int m) { return __shfl_xor_sync(0xffffffffu, x, m); }
 __device__ __forceinline__ cplx shfl_xor_c(cplx a, int m) { return mk(shfl_xor_d(a.re, m), shfl_xor_d(a.im, m)); }
+
+// Annealing noise (include/spgpe.h spgpe_set_annealing): element e of event k uses the
+// counter q = k * elems + e and the uniforms U(2q), U(2q+1) of the splitmix64 stream of `seed`,
+//   U(j) = (mix64(seed + (j+1) * 0x9E3779B97F4A7C15) >> 11) * 2^-53,   xi = sqrt(-2 ln(1 - u1)) e^{2 pi i u2},
+// and receives (amp / sqrt 2) xi.
+__device__ __forceinline__ unsigned long long mix64(unsigned long long z) {
+  z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ULL;
+  z ^= z >> 27; z *= 0x94D049BB133111EBULL;
+  z ^= z >> 31;
+  return z;
+}
+__device__ __forceinline__ double stream_uniform(unsigned long long seed, unsigned long long j) {
+  return (double)(mix64(seed + (j + 1ULL) * 0x9E3779B97F4A7C15ULL) >> 11) * (1.0 / 9007199254740992.0);
+}
+static __device__ __noinline__ cplx anneal_noise(const PassXArgs& a, unsigned long long elem) {
+  const unsigned long long q = (unsigned long long)a.anneal_event * a.anneal_elems + elem;
+  const double u1 = stream_uniform(a.anneal_seed, 2ULL * q), u2 = stream_uniform(a.anneal_seed, 2ULL * q + 1ULL);
+  const double r = (a.anneal_amp * 0.70710678118654752440) * sqrt(-2.0 * log1p(-u1));
+  double sn, cn;
+  sincos(6.283185307179586476925286766559 * u2, &sn, &cn);
+  return mk(r * cn, r * sn);
+}
 
 // Copy the three field rows of this CTA's LINES rows into shared memory ([field][line][x], working precision); a NULL
 // field is filled with zeros.  Every thread of the CTA takes part.  Rows (XS == 1) are contiguous: thread 0 issues one
@@ -116,7 +151,7 @@ __device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, siz
 // TIER: evaluation tier of su2.cuh, guaranteed by the caller for every point of the warp.
 template <int DT, int NX, int LINES, int MODE, int TIER, bool BZ0>
 __device__ __forceinline__ void real_space_tier(cplx* v, const PassXArgs& a, const void* fbuf, int line, int t, int c,
-                                                const LaneCoef& lc, double& sm, double& so) {
+                                                const LaneCoef& lc, double& sm, double& so, ObsSums& ob) {
   typedef Store<DT> St;
   typedef typename St::real real;
   constexpr int T = NX / 16;
@@ -160,8 +195,10 @@ __device__ __forceinline__ void real_space_tier(cplx* v, const PassXArgs& a, con
       apply_phase(m, o[i], pr, pi);
     }
     if (MODE == MODE_EPI) {
-      sm += fma(m.re, m.re, m.im * m.im);
-      so += fma(o[i].re, o[i].re, o[i].im * o[i].im);
+      const double rm = fma(m.re, m.re, m.im * m.im), ro = fma(o[i].re, o[i].re, o[i].im * o[i].im);
+      sm += rm;
+      so += ro;
+      if (a.want_obs) { ob.mm = fma(rm, rm, ob.mm); ob.oo = fma(ro, ro, ob.oo); ob.mo = fma(rm, ro, ob.mo); }
     }
     v[i] = m;
   }
@@ -193,21 +230,89 @@ __device__ __forceinline__ int row_tier(const cplx* v, const PassXArgs& a, const
   return 3;
 }
 
+// Nested split (su2.cuh): MODE_MID runs D(tau/2) X(tau) D(tau) X(tau) D(tau/2): the trailing D(tau/2) of step n and the
+// leading one of step n+1 see the same densities (a diagonal phase does not change them) and are one D(tau).
+template <int DT, int NX, int LINES, int MODE, bool FAST>
+__device__ __forceinline__ void real_space_nested(cplx* v, const PassXArgs& a, const void* fbuf, int line, int t, int c,
+                                                  const LaneCoef& lc, double& sm, double& so, ObsSums& ob) {
+  typedef Store<DT> St;
+  typedef typename St::real real;
+  constexpr int T = NX / 16;
+  const real* fV = reinterpret_cast<const real*>(fbuf) + line * NX + t + 8 * c * T;
+  const real* fO = fV + LINES * NX;
+  const real* fD = fO + LINES * NX;
+  const double tau = a.tau, th = 0.5 * a.tau;
+  cplx o[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) o[i] = shfl_xor_c(v[8 + i], 1);
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    cplx m = v[i], oo = o[i];
+    const double Vv = St::lds(fV, i * T);
+    const double hO = 0.5 * St::lds(fO, i * T);
+    const double hD = lc.hs * St::lds(fD, i * T);
+    if (a.imag) {
+      nested_diag<true, FAST>(m, oo, Vv, hD, th, lc);
+      nested_rot<true, FAST>(m, oo, hO, tau);
+      nested_diag<true, FAST>(m, oo, Vv, hD, th, lc);
+    } else {
+      nested_diag<false, FAST>(m, oo, Vv, hD, th, lc);
+      nested_rot<false, FAST>(m, oo, hO, tau);
+      if (MODE == MODE_MID) {
+        nested_diag<false, FAST>(m, oo, Vv, hD, tau, lc);
+        nested_rot<false, FAST>(m, oo, hO, tau);
+      }
+      nested_diag<false, FAST>(m, oo, Vv, hD, th, lc);
+    }
+    if (MODE == MODE_EPI) {
+      const double rm = fma(m.re, m.re, m.im * m.im), ro = fma(oo.re, oo.re, oo.im * oo.im);
+      sm += rm;
+      so += ro;
+      if (a.want_obs) { ob.mm = fma(rm, rm, ob.mm); ob.oo = fma(ro, ro, ob.oo); ob.mo = fma(rm, ro, ob.mo); }
+    }
+    v[i] = m;
+    o[i] = oo;
+  }
+#pragma unroll
+  for (int i = 0; i < 8; ++i) v[8 + i] = shfl_xor_c(o[i], 1);
+}
+
+// every phase argument of the nested split of this warp and row is small enough for the series
+__device__ __forceinline__ bool nested_fast(const cplx* v, const PassXArgs& a, const LaneCoef& lc) {
+  double nmax = 0.0;
+#pragma unroll
+  for (int n = 0; n < 16; ++n) nmax = fmax(nmax, fma(v[n].re, v[n].re, v[n].im * v[n].im));
+  const double NT = nmax + shfl_xor_d(nmax, 1);
+  // |d_c| <= max|V| + max|delta|/2 + (|ca| + |cb|)max NT; the longest diagonal factor is D(tau) (MODE_MID)
+  const double d = a.fmax[0] + 0.5 * a.fmax[2] +
+                   (fmax(fabs(lc.cam), fabs(lc.cao)) + fmax(fabs(lc.cbm), fabs(lc.cbo))) * NT;
+  const double x = a.tau * d, th = 0.5 * a.tau * a.fmax[1];
+  const bool ok = (x * x <= SPGPE_Z_FAST) && (th * th <= SPGPE_Z_FAST);  // NaN fails
+  return __all_sync(0xffffffffu, ok);
+}
+
 template <int DT, int NX, int LINES, int MODE>
 __device__ __forceinline__ void real_space(cplx* v, const PassXArgs& a, const void* fbuf, int line, int t, int c,
-                                           const LaneCoef& lc, double& sm, double& so) {
+                                           const LaneCoef& lc, double& sm, double& so, ObsSums& ob) {
+  if (a.nest) {
+    // in imaginary time the densities grow or shrink inside D; the bound above holds for the entering state only,
+    // so imaginary time takes the general path (libm exp either way)
+    if (!a.imag && nested_fast(v, a, lc)) real_space_nested<DT, NX, LINES, MODE, true>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    else real_space_nested<DT, NX, LINES, MODE, false>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    return;
+  }
   const bool bz0 = a.hc.cb_u == 0.0 && a.hc.cb_d == 0.0;
   const int tier = row_tier<MODE>(v, a, lc, bz0 && MODE == MODE_MID);
   if (bz0) {  // all g equal: b_z has no density term
-    if (tier == 0) real_space_tier<DT, NX, LINES, MODE, 0, true>(v, a, fbuf, line, t, c, lc, sm, so);
-    else if (tier == 1) real_space_tier<DT, NX, LINES, MODE, 1, true>(v, a, fbuf, line, t, c, lc, sm, so);
-    else if (tier == 2) real_space_tier<DT, NX, LINES, MODE, 2, true>(v, a, fbuf, line, t, c, lc, sm, so);
-    else real_space_tier<DT, NX, LINES, MODE, 3, true>(v, a, fbuf, line, t, c, lc, sm, so);
+    if (tier == 0) real_space_tier<DT, NX, LINES, MODE, 0, true>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    else if (tier == 1) real_space_tier<DT, NX, LINES, MODE, 1, true>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    else if (tier == 2) real_space_tier<DT, NX, LINES, MODE, 2, true>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    else real_space_tier<DT, NX, LINES, MODE, 3, true>(v, a, fbuf, line, t, c, lc, sm, so, ob);
   } else {
-    if (tier == 0) real_space_tier<DT, NX, LINES, MODE, 0, false>(v, a, fbuf, line, t, c, lc, sm, so);
-    else if (tier == 1) real_space_tier<DT, NX, LINES, MODE, 1, false>(v, a, fbuf, line, t, c, lc, sm, so);
-    else if (tier == 2) real_space_tier<DT, NX, LINES, MODE, 2, false>(v, a, fbuf, line, t, c, lc, sm, so);
-    else real_space_tier<DT, NX, LINES, MODE, 3, false>(v, a, fbuf, line, t, c, lc, sm, so);
+    if (tier == 0) real_space_tier<DT, NX, LINES, MODE, 0, false>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    else if (tier == 1) real_space_tier<DT, NX, LINES, MODE, 1, false>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    else if (tier == 2) real_space_tier<DT, NX, LINES, MODE, 2, false>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    else real_space_tier<DT, NX, LINES, MODE, 3, false>(v, a, fbuf, line, t, c, lc, sm, so, ob);
   }
 }
 
@@ -237,6 +342,7 @@ pass_x_kernel(const PassXArgs a) {
   double2* buf = smem + (size_t)line * (P::PTS * 2);
   const int ngroups = a.ny / LINES;
   double sm = 0.0, so = 0.0;  // sums of |own component|^2 and |other component|^2 over this lane's points
+  ObsSums ob = {0.0, 0.0, 0.0};
   const LaneCoef lc = lane_coef(a.hc, c);
   const int flip = c ? (int)0x80000000 : 0;  // the odd lane keeps its points rotated by 8 (twiddle())
   cplx v[16];
@@ -320,7 +426,7 @@ pass_x_kernel(const PassXArgs a) {
     }
   };
 
-  __shared__ double red[2][32];
+  __shared__ double red[5][32];
   __shared__ int next_s[2];  // group this CTA takes next (written by thread 0, double-buffered over iterations)
   int it = 0;
   TL_DECL(8);
@@ -339,6 +445,18 @@ pass_x_kernel(const PassXArgs a) {
       const double s = a.scale[c];
 #pragma unroll
       for (int n = 0; n < 16; ++n) v[n] = mk(v[n].re * s, v[n].im * s);
+    }
+    if (MODE == MODE_PRO && a.anneal_event > 0) {
+#pragma unroll 1
+      for (int n = 0; n < 16; ++n) {
+        // register n holds point t + ((n + 8c) mod 16) T of the line (same index as the load above)
+        const unsigned long long e = (unsigned long long)(lbase + (size_t)(t + ((n + 8 * c) & 15) * T) * S) * 2ULL + c;
+        const cplx z = anneal_noise(a, e);
+        // v[n] with a run-time n would leave the registers: select instead
+#pragma unroll
+        for (int k = 0; k < 16; ++k)
+          if (k == n) v[k] = v[k] + z;
+      }
     }
     __syncthreads();  // every thread has taken its staged values: the buffers may be overwritten
     TL_MARK(0);
@@ -360,9 +478,9 @@ pass_x_kernel(const PassXArgs a) {
       // complete on the mbarrier every thread has just waited on
       if (!FBULK || a.V == nullptr || a.Om == nullptr || a.De == nullptr) __syncthreads();
       TL_MARK(2);
-      real_space<DT, NX, LINES, MODE>(v, a, smem, line, t, c, lc, sm, so);
+      real_space<DT, NX, LINES, MODE>(v, a, smem, line, t, c, lc, sm, so, ob);
       TL_MARK(3);
-      if (MODE == MODE_EPI && a.want_norm) {
+      if (MODE == MODE_EPI && (a.want_norm || a.want_obs)) {
         // norm partials of this row group, one slot per group: the sums do not depend on which CTA took the group,
         // so the reduction order (and every imaginary-time result) is the same from run to run.  Each lane summed
         // its own and the other component over its 8 points: sort into (up, down) first.
@@ -375,13 +493,26 @@ pass_x_kernel(const PassXArgs a) {
           sd += shfl_xor_d(sd, m);
         }
         if ((tid & 31) == 0) { red[0][tid >> 5] = su; red[1][tid >> 5] = sd; }
+        if (a.want_obs) {  // rho_up^2, rho_dn^2, rho_up rho_dn of the group (same sorting, same fixed order)
+          double quu = c ? ob.oo : ob.mm, qdd = c ? ob.mm : ob.oo, qud = ob.mo;
+          ob.mm = ob.oo = ob.mo = 0.0;
+#pragma unroll
+          for (int m = 16; m >= 1; m >>= 1) {
+            quu += shfl_xor_d(quu, m);
+            qdd += shfl_xor_d(qdd, m);
+            qud += shfl_xor_d(qud, m);
+          }
+          if ((tid & 31) == 0) { red[2][tid >> 5] = quu; red[3][tid >> 5] = qdd; red[4][tid >> 5] = qud; }
+        }
       }
       __syncthreads();
-      if (MODE == MODE_EPI && a.want_norm && tid == 0) {
-        double s0 = 0.0, s1 = 0.0;
-        for (int i = 0; i < NTHR / 32; ++i) { s0 += red[0][i]; s1 += red[1][i]; }
-        a.partial[2 * grp] = s0;
-        a.partial[2 * grp + 1] = s1;
+      if (MODE == MODE_EPI && (a.want_norm || a.want_obs) && tid == 0) {
+        const int nk = a.want_obs ? 5 : 2;
+        for (int k = 0; k < nk; ++k) {
+          double s0 = 0.0;
+          for (int i = 0; i < NTHR / 32; ++i) s0 += red[k][i];
+          a.partial[(size_t)a.pstride * grp + k] = s0;
+        }
       }
     }
 
@@ -425,8 +556,8 @@ pass_x_kernel(const PassXArgs a) {
       if (last_s) {
         double x0 = 0.0, x1 = 0.0;
         for (int b = tid; b < ngroups; b += NTHR) {
-          x0 += __ldcg(a.partial + 2 * (size_t)b);
-          x1 += __ldcg(a.partial + 2 * (size_t)b + 1);
+          x0 += __ldcg(a.partial + (size_t)a.pstride * b);
+          x1 += __ldcg(a.partial + (size_t)a.pstride * b + 1);
         }
 #pragma unroll
         for (int m = 16; m >= 1; m >>= 1) {

@@ -11,6 +11,8 @@
 //   YMODE_ENERGY : psi^(k_x, y) -> F_y -> sum (Kx_c(k_x) + Ky(k_y)) |psi^|^2 -> partial[CTA]
 //   YMODE_FWDONLY: psi^(k_x, y) -> F_y -> psi^(k_x, k_y) in stored order          (split transforms, api.cu)
 //   YMODE_INVONLY: psi^(k_x, k_y) in stored order -> F_y^-1 -> psi^(k_x, y)
+//   YMODE_STEP_OBS: YMODE_STEP that also leaves, per CTA, the k-space sums of include/spgpe.h spgpe_step_observe
+//                  (sum |psi^_c|^2, sum K_c |psi^_c|^2, sum k_x |psi^_c|^2, taken in front of the k-space factor)
 #pragma once
 #include <cuda.h>
 
@@ -18,7 +20,7 @@
 
 namespace spgpe {
 
-enum { YMODE_STEP = 0, YMODE_ENERGY = 1, YMODE_FWDONLY = 2, YMODE_INVONLY = 3 };
+enum { YMODE_STEP = 0, YMODE_ENERGY = 1, YMODE_FWDONLY = 2, YMODE_INVONLY = 3, YMODE_STEP_OBS = 4 };
 
 struct PassYArgs {
   void* psi;            // [NY][nx][2]
@@ -27,7 +29,8 @@ struct PassYArgs {
   const double2* exk;   // [2][nx] k_x phase in the row pass's stored order (YMODE_STEP), or NULL (none applied here)
   const double* Kx;     // [2][nx] (k_x +- k_L)^2/2 in the row pass's stored order (YMODE_ENERGY)
   const double* Ky;     // [NY] k_y^2/2 in stored order (YMODE_ENERGY)
-  double* partial;      // [gridDim.x] sum over this CTA's columns (YMODE_ENERGY)
+  double* partial;      // [gridDim.x] sum over this CTA's columns (YMODE_ENERGY); [gridDim.x][6] (YMODE_STEP_OBS)
+  const double* kxv;    // [nx] k_x in the row pass's stored order (YMODE_STEP_OBS)
   int nx;
   int* sched;           // [2] device: work counter (common.cuh, sched_next)
   // psi as a 2-D tensor [NY rows][4 nx reals], box = [min(NY, 256) rows][4 LINES reals]: the columns of a group
@@ -65,6 +68,8 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
   extern __shared__ __align__(128) double2 smem[];
   constexpr int T = P::T;
   constexpr int NTHR = LINES * (NY / 8);
+  constexpr bool STEP = (YMODE == YMODE_STEP || YMODE == YMODE_STEP_OBS);
+  constexpr bool OBS = (YMODE == YMODE_STEP_OBS);
   const int tid = threadIdx.x;
   const int c = tid & 1;
   const int line = (tid >> 1) % LINES;
@@ -72,9 +77,10 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
   double2* buf = smem + (size_t)line * (YLayout<NY, LINES>::LINE_PTS * 2);
   double2* twS = smem + SM::EBUF;
   const double2* ey = a.eyk;
+  double om = 0.0, ot = 0.0, op = 0.0;  // OBS: sums of |z|^2, K_c |z|^2, k_x |z|^2 of this thread's component
   pdl_launch_dependents();
   copy_table_async(twS, a.tw, SM::TW, tid, NTHR);
-  if (YMODE == YMODE_STEP && SM::EY_SMEM) {
+  if (STEP && SM::EY_SMEM) {
     double2* eyS = twS + SM::TW;
     copy_table_async(eyS, a.eyk, NY, tid, NTHR);
     ey = eyS;
@@ -120,7 +126,7 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
     const size_t e0 = ((size_t)t * nx + col) * 2 + c;  // element (row t, column col, component c)
     // k_x phase of this column and component (see pass_y_db_kernel); requested now, used after the forward transform
     double2 exv = make_double2(1.0, 0.0);
-    if (YMODE == YMODE_STEP && a.exk != nullptr) exv = __ldg(a.exk + (size_t)c * nx + col);
+    if (STEP && a.exk != nullptr) exv = __ldg(a.exk + (size_t)c * nx + col);
     // the next group is requested now and published before the last barrier of this iteration (latency hidden)
     int nxt_req = 0;
     if (tid == 0) {
@@ -146,8 +152,24 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
 
     if (YMODE != YMODE_INVONLY) line_fft_fwd<NY>(buf, twS, t, c, v);
 
-    if (YMODE == YMODE_STEP || YMODE == YMODE_INVONLY) {
-      if (YMODE == YMODE_STEP) {
+    if (OBS) {
+      const double kxc = a.Kx[(size_t)c * nx + col], kx1 = a.kxv[col];
+      double m0 = 0.0, t0 = 0.0;
+#pragma unroll
+      for (int g = 0; g < P::G; ++g)
+#pragma unroll
+        for (int s = 0; s < P::RL; ++s) {
+          const cplx z = v[g * P::RL + s];
+          const double r = fma(z.re, z.re, z.im * z.im);
+          m0 += r;
+          t0 = fma(kxc + a.Ky[(t + g * T) + (NY / P::RL) * s], r, t0);
+        }
+      om += m0;
+      ot += t0;
+      op = fma(kx1, m0, op);
+    }
+    if (STEP || YMODE == YMODE_INVONLY) {
+      if (STEP) {
 #pragma unroll
       for (int g = 0; g < P::G; ++g)
 #pragma unroll
@@ -197,6 +219,24 @@ pass_y_kernel(const __grid_constant__ PassYArgs a) {
   }
   if (tid == 0) sched_finish(a.sched);
 
+  if (OBS) {
+    // component c sits in the lanes of parity c: reduce over the lanes of equal parity, then over the warps
+    __shared__ double redo[6][32];
+#pragma unroll
+    for (int m = 16; m >= 2; m >>= 1) {
+      om += __shfl_xor_sync(0xffffffffu, om, m);
+      ot += __shfl_xor_sync(0xffffffffu, ot, m);
+      op += __shfl_xor_sync(0xffffffffu, op, m);
+    }
+    const int w = tid >> 5, nw = (blockDim.x + 31) >> 5;
+    if ((tid & 31) < 2) { redo[c][w] = om; redo[2 + c][w] = ot; redo[4 + c][w] = op; }
+    __syncthreads();
+    if (tid < 6) {
+      double s0 = 0.0;
+      for (int i = 0; i < nw; ++i) s0 += redo[tid][i];
+      a.partial[(size_t)blockIdx.x * 6 + tid] = s0;
+    }
+  }
   if (YMODE == YMODE_ENERGY) {
     __shared__ double red[32];
 #pragma unroll

@@ -171,4 +171,44 @@ __device__ __forceinline__ void apply_phase(cplx& up, cplx& dn, double pr, doubl
   dn = cmul(dn, mk(pr, pi));
 }
 
+// ---- nested second-order split of the real-space part (R-15) -----------
+//   R_nested(tau) = D(tau/2) X(tau) D(tau/2),
+// D(s): psi_c <- e^{-i s d_c} psi_c with d_m = a + b_z, d_o = a - b_z in the lane's (mine, other) basis (a, b_z as in
+// LaneCoef above, densities of the psi that enters D); X(s) = exp(-i s (Omega/2) sigma_x).  Imaginary time: e^{-s d_c},
+// cosh / sinh.  FAST: every phase argument x of the warp satisfies x^2 <= SPGPE_Z_FAST (series), else libm.
+template <bool IMAG, bool FAST>
+__device__ __forceinline__ void nested_diag(cplx& m, cplx& o, double V, double hDs, double s, const LaneCoef& lc) {
+  const double nm = fma(m.re, m.re, m.im * m.im);
+  const double no = fma(o.re, o.re, o.im * o.im);
+  const double a = fma(lc.cam, nm, fma(lc.cao, no, V));
+  const double bz = fma(lc.cbm, nm, fma(lc.cbo, no, hDs));
+  const double dm = a + bz, dn = a - bz;
+  if (IMAG) {
+    const double em = exp(-dm * s), eo = exp(-dn * s);
+    m = mk(m.re * em, m.im * em);
+    o = mk(o.re * eo, o.im * eo);
+  } else {
+    double pr, pi;
+    phase_eval<FAST ? 2 : 3>(dm * s, pr, pi);
+    m = cmul(m, mk(pr, pi));
+    phase_eval<FAST ? 2 : 3>(dn * s, pr, pi);
+    o = cmul(o, mk(pr, pi));
+  }
+}
+template <bool IMAG, bool FAST>
+__device__ __forceinline__ void nested_rot(cplx& m, cplx& o, double hO, double s) {
+  const double th = hO * s;
+  double C, S;
+  cs_eval<IMAG, FAST ? 2 : 3>(IMAG ? th * th : -(th * th), C, S);
+  const double sn = th * S;  // sin(th) or sinh(th)
+  const cplx m0 = m;
+  if (IMAG) {
+    m = mk(fma(C, m.re, -(sn * o.re)), fma(C, m.im, -(sn * o.im)));
+    o = mk(fma(C, o.re, -(sn * m0.re)), fma(C, o.im, -(sn * m0.im)));
+  } else {  // -i sn (x + i y) = sn y - i sn x
+    m = mk(fma(C, m.re, sn * o.im), fma(C, m.im, -(sn * o.re)));
+    o = mk(fma(C, o.re, sn * m0.im), fma(C, o.im, -(sn * m0.re)));
+  }
+}
+
 }  // namespace spgpe

@@ -1,0 +1,171 @@
+"""Parity of the SURVEY.md 8(f) rows with the oracle, through the C ABI: the nested second-order real-space split
+(spgpe_set_real_space_split), the annealing noise generated inside the row pass (spgpe_set_annealing) and the
+observables accumulated inside the passes of the last step (spgpe_step_observe).  Same tolerances as
+tests/test_gpu_parity.py (BASELINE.json): relative L2 of psi <= 1e-10 (complex128), 1e-4 (complex64 storage), with the
+element-wise bound beside it; observables within 1e-9 relative (complex128).
+"""
+import numpy as np
+import pytest
+
+import oracle as orc
+import workloads as wl
+from test_gpu_parity import TOL_C128, TOL_C64, assert_parity, make_solver, random_problem, sp  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+TOL_OBS = 1e-9
+
+
+# ---------------------------------------------------------------- NEXT-1
+@pytest.mark.parametrize("nx,ny", [(64, 64), (256, 128), (128, 1024), (2048, 64), (512, 512)])
+def test_nested_split_real_time_matches_oracle(sp, nx, ny):
+    psi, V, Om, De, p, _ = random_problem(nx, ny, seed=3 * nx + ny)
+    p.rs_split = 1
+    h = make_solver(sp, psi, V, Om, De, p)
+    sp.spgpe_set_real_space_split(h, sp.SPGPE_RS_NESTED)
+    n, dt = 4, 2e-3
+    sp.spgpe_step(h, n, dt, 0)   # PRO, MID x 3 (the merged D(tau) of the kernel), EPI
+    ref = orc.step(psi, V, Om, De, p, n, dt, 0)
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C128)
+    sp.spgpe_step(h, 1, -dt, 0)  # PRO + EPI only, negative dt
+    ref = orc.step(ref, V, Om, De, p, 1, -dt, 0)
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C128)
+    # switching back gives the single exponential again
+    sp.spgpe_set_real_space_split(h, sp.SPGPE_RS_EXPONENTIAL)
+    p.rs_split = 0
+    sp.spgpe_step(h, 2, dt, 0)
+    assert_parity(sp.spgpe_get_psi_host(h), orc.step(ref, V, Om, De, p, 2, dt, 0), TOL_C128)
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_nested_split_imaginary_time_matches_oracle(sp, mode):
+    psi, V, Om, De, p, _ = random_problem(256, 64, seed=77)
+    p.rs_split, p.norm_mode = 1, mode
+    h = make_solver(sp, psi, V, Om, De, p)
+    sp.spgpe_set_real_space_split(h, sp.SPGPE_RS_NESTED)
+    sp.spgpe_step(h, 5, 1e-3, 1)
+    ref = orc.step(psi, V, Om, De, p, 5, 1e-3, 1)
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C128)
+
+
+def test_nested_split_general_path_large_arguments(sp):
+    """Phase arguments far outside the series range (libm path), both signs of dt."""
+    psi, V, Om, De, p, _ = random_problem(128, 64, seed=5)
+    p.rs_split = 1
+    V = 40.0 * V
+    Om = 30.0 * Om
+    h = make_solver(sp, psi, V, Om, De, p)
+    sp.spgpe_set_real_space_split(h, sp.SPGPE_RS_NESTED)
+    sp.spgpe_step(h, 3, 0.05, 0)
+    ref = orc.step(psi, V, Om, De, p, 3, 0.05, 0)
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C128)
+
+
+def test_nested_split_config2_proxy_and_c64(sp):
+    """Config 2's recipe (Omega != 0, unequal g: the case the nested split exists for), 200 steps; complex64 storage."""
+    w = wl.make_workload(2, n=128)
+    p = orc.params_of(w, rs_split=1)
+    h = sp.from_workload(w)
+    sp.spgpe_set_real_space_split(h, sp.SPGPE_RS_NESTED)
+    sp.spgpe_step(h, 200, 5e-4, 0)
+    ref = orc.step(w.psi0, w.V, w.Omega, w.delta, p, 200, 5e-4, 0)
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C128)
+    # complex64 storage: inputs rounded to fp32 first, those values to both sides (R-14)
+    f32 = lambda a: None if a is None else np.ascontiguousarray(a, dtype=np.float32).astype(np.float64)
+    psi32 = np.ascontiguousarray(w.psi0, dtype=np.complex64).astype(np.complex128)
+    h = make_solver(sp, psi32, f32(w.V), f32(w.Omega), f32(w.delta), p, dtype="c64")
+    sp.spgpe_set_real_space_split(h, sp.SPGPE_RS_NESTED)
+    sp.spgpe_step(h, 20, 5e-4, 0)
+    ref = orc.step(psi32, f32(w.V), f32(w.Omega), f32(w.delta), p, 20, 5e-4, 0)
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C64)
+
+
+# ---------------------------------------------------------------- NEXT-3
+@pytest.mark.parametrize("nx,ny", [(64, 64), (256, 128), (128, 512), (2048, 64)])
+def test_annealed_imaginary_time_matches_oracle(sp, nx, ny):
+    psi, V, Om, De, p, _ = random_problem(nx, ny, seed=11 + nx)
+    h = make_solver(sp, psi, V, Om, De, p)
+    every, amp, seed = 2, 0.05, 0xDEADBEEFCAFE1234
+    sp.spgpe_set_annealing(h, every, amp, seed)
+    t = orc.norm(psi, p)
+    sp.spgpe_step(h, 3, 1e-3, 1)   # steps 0, 1, 2: event 1 enters step 2
+    ref = orc.step_anneal(psi, V, Om, De, p, 3, 1e-3, every, amp, seed)
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C128)
+    # the noise is really there: the plain run differs by far more than the tolerance
+    assert np.abs(ref - orc.step(psi, V, Om, De, p, 3, 1e-3, 1)).max() > 1e-4
+    sp.spgpe_step(h, 4, 1e-3, 1)   # steps 3..6 of the same schedule: events 2 and 3
+    ref = orc.step_anneal(ref, V, Om, De, p, 4, 1e-3, every, amp, seed, first_step=3, targets=t)
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C128)
+    # switched off: plain imaginary time again
+    sp.spgpe_set_annealing(h, 0, 0.0, 0)
+    sp.spgpe_step(h, 2, 1e-3, 1)
+    assert_parity(sp.spgpe_get_psi_host(h), orc.step(ref, V, Om, De, p, 2, 1e-3, 1, targets=t), TOL_C128)
+
+
+def test_annealing_noise_alone_is_the_stated_stream(sp):
+    """One step of tiny d tau on a flat state with no fields: psi_out - psi_in is (up to the O(d tau) drift and the
+    renormalisation) the noise itself; compared with the oracle's generator element by element at amplitude 1."""
+    nx, ny = 128, 64
+    p = orc.params(nx, ny, 8.0, 8.0)
+    psi = np.full((ny, nx, 2), 0.5 + 0.0j)
+    h = make_solver(sp, psi, None, None, None, p)
+    sp.spgpe_set_annealing(h, 1, 1.0, 987654321)
+    sp.spgpe_step(h, 2, 1e-9, 1)   # step 1 receives event 1
+    ref = orc.step_anneal(psi, None, None, None, p, 2, 1e-9, 1, 1.0, 987654321)
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C128)
+
+
+# ---------------------------------------------------------------- NEXT-2
+@pytest.mark.parametrize("nx,ny", [(64, 64), (256, 128), (128, 1024), (2048, 64), (1024, 1024)])
+@pytest.mark.parametrize("imag", [0, 1])
+def test_step_observe_matches_oracle(sp, nx, ny, imag):
+    psi, V, Om, De, p, _ = random_problem(nx, ny, seed=21 + nx + imag)
+    h = make_solver(sp, psi, V, Om, De, p)
+    n, dt = 3, 1e-3
+    got = sp.spgpe_step_observe(h, n, dt, imag)
+    ref, o_r, o_k = orc.step_observe(psi, V, Om, De, p, n, dt, imag)
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C128)
+    want = np.concatenate([o_r, o_k])
+    scale = np.array([want[0], want[1], want[2], want[3], want[4], 1.0,
+                      want[6], want[7], want[8], want[9], max(abs(want[10]), want[6]), max(abs(want[11]), want[7])])
+    assert (np.abs(got - want) <= TOL_OBS * np.abs(scale)).all(), (got, want)
+    # n = 1 (prologue + observed column pass + observed closing pass only)
+    got1 = sp.spgpe_step_observe(h, 1, dt, imag)
+    t = orc.norm(psi, p)
+    ref1, r1, k1 = orc.step_observe(ref, V, Om, De, p, 1, dt, imag, targets=t)
+    assert_parity(sp.spgpe_get_psi_host(h), ref1, TOL_C128)
+    assert (np.abs(got1 - np.concatenate([r1, k1])) <= TOL_OBS * np.abs(scale)).all()
+
+
+def test_step_observe_with_nested_split_and_c64(sp):
+    w = wl.make_workload(2, n=256)
+    p = orc.params_of(w, rs_split=1)
+    h = sp.from_workload(w)
+    sp.spgpe_set_real_space_split(h, sp.SPGPE_RS_NESTED)
+    got = sp.spgpe_step_observe(h, 5, 5e-4, 0)
+    ref, o_r, o_k = orc.step_observe(w.psi0, w.V, w.Omega, w.delta, p, 5, 5e-4, 0)
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C128)
+    want = np.concatenate([o_r, o_k])
+    np.testing.assert_allclose(got[:10], want[:10], rtol=TOL_OBS, atol=TOL_OBS)
+    np.testing.assert_allclose(got[10:], want[10:], rtol=0, atol=TOL_OBS * want[6])
+    # complex64 storage: observables follow the fp32-rounded state
+    p0 = orc.params_of(w)
+    f32 = lambda a: None if a is None else np.ascontiguousarray(a, dtype=np.float32).astype(np.float64)
+    psi32 = np.ascontiguousarray(w.psi0, dtype=np.complex64).astype(np.complex128)
+    h = make_solver(sp, psi32, f32(w.V), f32(w.Omega), f32(w.delta), p0, dtype="c64")
+    got = sp.spgpe_step_observe(h, 3, 5e-4, 0)
+    ref, o_r, o_k = orc.step_observe(psi32, f32(w.V), f32(w.Omega), f32(w.delta), p0, 3, 5e-4, 0)
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C64)
+    np.testing.assert_allclose(got[:5], o_r[:5], rtol=1e-5)
+    np.testing.assert_allclose(got[6:10], o_k[:4], rtol=1e-5)
+
+
+def test_step_observe_argument_errors(sp):
+    psi, V, Om, De, p, _ = random_problem(64, 64, seed=1)
+    h = make_solver(sp, psi, V, Om, De, p)
+    with pytest.raises(sp.SpgpeError):
+        sp.spgpe_step_observe(h, 0, 1e-3, 0)
+    with pytest.raises(sp.SpgpeError):
+        sp.spgpe_set_real_space_split(h, 7)
+    with pytest.raises(sp.SpgpeError):
+        sp.spgpe_set_annealing(h, -1, 0.1, 0)
