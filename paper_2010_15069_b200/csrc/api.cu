@@ -499,8 +499,8 @@ static int step_impl(spgpe_handle h, int n, double dt, int imag, bool obs) {
     for (int s = 1; s <= n; ++s) {
       if (s < n) CK(kspace_part(h, ya));
       else CK(last_kspace());
-      if (s == n && obs) { xa.want_obs = 1; xa.pstride = 8; }
-      CK(dispatch_x(h, s < n ? MODE_MID : MODE_EPI, xa));
+      if (s == n && obs) xa.pstride = 8;
+      CK(dispatch_x(h, s < n ? MODE_MID : (obs ? MODE_EPI_OBS : MODE_EPI), xa));
     }
   } else {
     for (int s = 0; s < n; ++s) {
@@ -510,8 +510,9 @@ static int step_impl(spgpe_handle h, int n, double dt, int imag, bool obs) {
       CK(dispatch_x(h, MODE_PRO, xa));
       if (s + 1 < n) CK(kspace_part(h, ya));
       else CK(last_kspace());
-      if (s + 1 == n && obs) { xa.want_obs = 1; xa.pstride = 8; }
-      CK(dispatch_x(h, MODE_EPI, xa));  // also writes the rescale factors (last CTA)
+      const bool last_obs = obs && s + 1 == n;
+      if (last_obs) xa.pstride = 8;
+      CK(dispatch_x(h, last_obs ? MODE_EPI_OBS : MODE_EPI, xa));  // also writes the rescale factors (last CTA)
     }
     h->imag_steps += n;
     h->launches++;

@@ -66,10 +66,10 @@ cudaError_t launch_pdl(K kernel, int grid, int threads, size_t smem, cudaStream_
 }
 
 // grid_out: number of CTAs launched (= rows of PassXArgs::partial written by MODE_EPI)
-template <int DT, int N, int MODE, int XS>
+template <int DT, int N, int MODE, int XS, bool NEST>
 cudaError_t launch_x_xs(const PassXArgs& a, int ny, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
   constexpr int L = Lines<N>::X;
-  auto k = pass_x_kernel<DT, N, L, MODE, XS>;
+  auto k = pass_x_kernel<DT, N, L, MODE, XS, NEST>;
   constexpr size_t smem = XSmem<N, L>::BYTES;
   static int cache[SPGPE_MAX_DEVICES] = {};
   int resident = 0;
@@ -83,8 +83,13 @@ cudaError_t launch_x_xs(const PassXArgs& a, int ny, cudaStream_t s, const Launch
 
 template <int DT, int N, int MODE>
 cudaError_t launch_x(const PassXArgs& a, int ny, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
-  return a.xs == 1 ? launch_x_xs<DT, N, MODE, 1>(a, ny, s, env, grid_out)
-                   : launch_x_xs<DT, N, MODE, 2>(a, ny, s, env, grid_out);
+  if constexpr (MODE != MODE_FWD) {  // the transform-only mode has no real-space part
+    if (a.nest)
+      return a.xs == 1 ? launch_x_xs<DT, N, MODE, 1, true>(a, ny, s, env, grid_out)
+                       : launch_x_xs<DT, N, MODE, 2, true>(a, ny, s, env, grid_out);
+  }
+  return a.xs == 1 ? launch_x_xs<DT, N, MODE, 1, false>(a, ny, s, env, grid_out)
+                   : launch_x_xs<DT, N, MODE, 2, false>(a, ny, s, env, grid_out);
 }
 
 template <int DT, int N, int YMODE>
@@ -171,6 +176,7 @@ cudaError_t launch_y_step(const PassYArgs& a, cudaStream_t s, const LaunchEnv& e
         case MODE_PRO: return launch_x<0, N_, MODE_PRO>(a, ny, s, env, g);                               \
         case MODE_MID: return launch_x<0, N_, MODE_MID>(a, ny, s, env, g);                               \
         case MODE_EPI: return launch_x<0, N_, MODE_EPI>(a, ny, s, env, g);                               \
+        case MODE_EPI_OBS: return launch_x<0, N_, MODE_EPI_OBS>(a, ny, s, env, g);                       \
         default: return launch_x<0, N_, MODE_FWD>(a, ny, s, env, g);                                     \
       }                                                                                          \
     }                                                                                            \
@@ -178,6 +184,7 @@ cudaError_t launch_y_step(const PassYArgs& a, cudaStream_t s, const LaunchEnv& e
       case MODE_PRO: return launch_x<1, N_, MODE_PRO>(a, ny, s, env, g);                                 \
       case MODE_MID: return launch_x<1, N_, MODE_MID>(a, ny, s, env, g);                                 \
       case MODE_EPI: return launch_x<1, N_, MODE_EPI>(a, ny, s, env, g);                                 \
+      case MODE_EPI_OBS: return launch_x<1, N_, MODE_EPI_OBS>(a, ny, s, env, g);                         \
       default: return launch_x<1, N_, MODE_FWD>(a, ny, s, env, g);                                       \
     }                                                                                            \
   }                                                                                              \

@@ -7,6 +7,7 @@
 //   MODE_PRO : psi(x) -> [scale] -> R(tau) -> F_x -> psi^(k_x)                          (first half of a step)
 //   MODE_MID : psi^(k_x) -> F_x^-1 -> R(tau) R(tau) -> F_x -> psi^(k_x)                  (real time, steps n | n+1)
 //   MODE_EPI : psi^(k_x) -> F_x^-1 -> R(tau) -> [norm partials] -> psi(x)              (second half of a step)
+//   MODE_EPI_OBS: MODE_EPI with the observables' partial sums
 //   MODE_FWD : src psi(x) -> F_x -> dst psi^(k_x)                                      (energy only)
 // The two half-steps of MODE_MID are two evaluations with refreshed densities (R-6); only their scalar phases
 // e^{-i a1 tau} e^{-i a2 tau} are merged into one (unit-modulus phases do not change densities).  One exact exception:
@@ -17,7 +18,10 @@
 
 namespace spgpe {
 
-enum { MODE_PRO = 0, MODE_MID = 1, MODE_EPI = 2, MODE_FWD = 3 };
+enum { MODE_PRO = 0, MODE_MID = 1, MODE_EPI = 2, MODE_FWD = 3, MODE_EPI_OBS = 4 };
+// MODE_EPI_OBS: MODE_EPI that also sums rho_up^2, rho_dn^2, rho_up rho_dn (spgpe_step_observe); its own instantiation,
+// so that the closing pass of every imaginary-time step keeps its register budget
+__host__ __device__ constexpr bool mode_is_epi(int m) { return m == MODE_EPI || m == MODE_EPI_OBS; }
 
 struct PassXArgs {
   const void* src;       // psi in   [ny][NX][2]
@@ -27,7 +31,7 @@ struct PassXArgs {
   const void* De;
   const double2* tw;     // twiddles of NX
   const double* scale;   // [2] per-component factor applied at load (MODE_PRO, imaginary time) or NULL
-  double* partial;       // [ny / LINES][pstride] sums of every row group (MODE_EPI with want_norm or want_obs)
+  double* partial;       // [ny / LINES][pstride] sums of every row group (MODE_EPI with want_norm, MODE_EPI_OBS)
   double tau;            // half-step size dt/2
   HalfCoef hc;
   int imag;
@@ -41,8 +45,7 @@ struct PassXArgs {
   int norm_mode;         // SPGPE_NORM_PER_COMPONENT | SPGPE_NORM_TOTAL
   const double* fmax;    // [3] device: max |V|, max |Omega|, max |delta| over the grid (tier bounds)
   int nest;              // 1: nested second-order split D(tau/2) X(tau) D(tau/2) of the real-space part (su2.cuh)
-  int want_obs;          // MODE_EPI: five partial sums per row group (norms, rho_up^2, rho_dn^2, rho_up rho_dn)
-  int pstride;           // doubles per row group in `partial`: 2 (norms only) or 8 (want_obs)
+  int pstride;           // doubles per row group in `partial`: 2 (norms only) or 8 (MODE_EPI_OBS: five sums)
   // annealing (MODE_PRO): noise of event `anneal_event` (0: none) added to the order parameter at load
   long long anneal_event;
   unsigned long long anneal_seed;
@@ -51,7 +54,7 @@ struct PassXArgs {
   int dbg;               // experiment switches (bit 0: psi rows by bulk copy, 1: field rows by per-thread cp.async instead of bulk copies, 2: early L2 prefetch)
 };
 
-// observables of the final state (MODE_EPI with want_obs): sums of rho_m^2, rho_o^2, rho_m rho_o over the lane's points
+// observables of the final state (MODE_EPI_OBS): sums of rho_m^2, rho_o^2, rho_m rho_o over the lane's points
 struct ObsSums {
   double mm, oo, mo;
 };
@@ -194,11 +197,11 @@ __device__ __forceinline__ void real_space_tier(cplx* v, const PassXArgs& a, con
       phase_eval<TIER>(a1 * tau, pr, pi);
       apply_phase(m, o[i], pr, pi);
     }
-    if (MODE == MODE_EPI) {
+    if (mode_is_epi(MODE)) {
       const double rm = fma(m.re, m.re, m.im * m.im), ro = fma(o[i].re, o[i].re, o[i].im * o[i].im);
       sm += rm;
       so += ro;
-      if (a.want_obs) { ob.mm = fma(rm, rm, ob.mm); ob.oo = fma(ro, ro, ob.oo); ob.mo = fma(rm, ro, ob.mo); }
+      if (MODE == MODE_EPI_OBS) { ob.mm = fma(rm, rm, ob.mm); ob.oo = fma(ro, ro, ob.oo); ob.mo = fma(rm, ro, ob.mo); }
     }
     v[i] = m;
   }
@@ -264,11 +267,11 @@ __device__ __forceinline__ void real_space_nested(cplx* v, const PassXArgs& a, c
       }
       nested_diag<false, FAST>(m, oo, Vv, hD, th, lc);
     }
-    if (MODE == MODE_EPI) {
+    if (mode_is_epi(MODE)) {
       const double rm = fma(m.re, m.re, m.im * m.im), ro = fma(oo.re, oo.re, oo.im * oo.im);
       sm += rm;
       so += ro;
-      if (a.want_obs) { ob.mm = fma(rm, rm, ob.mm); ob.oo = fma(ro, ro, ob.oo); ob.mo = fma(rm, ro, ob.mo); }
+      if (MODE == MODE_EPI_OBS) { ob.mm = fma(rm, rm, ob.mm); ob.oo = fma(ro, ro, ob.oo); ob.mo = fma(rm, ro, ob.mo); }
     }
     v[i] = m;
     o[i] = oo;
@@ -291,10 +294,10 @@ __device__ __forceinline__ bool nested_fast(const cplx* v, const PassXArgs& a, c
   return __all_sync(0xffffffffu, ok);
 }
 
-template <int DT, int NX, int LINES, int MODE>
+template <int DT, int NX, int LINES, int MODE, bool NEST>
 __device__ __forceinline__ void real_space(cplx* v, const PassXArgs& a, const void* fbuf, int line, int t, int c,
                                            const LaneCoef& lc, double& sm, double& so, ObsSums& ob) {
-  if (a.nest) {
+  if constexpr (NEST) {
     // in imaginary time the densities grow or shrink inside D; the bound above holds for the entering state only,
     // so imaginary time takes the general path (libm exp either way)
     if (!a.imag && nested_fast(v, a, lc)) real_space_nested<DT, NX, LINES, MODE, true>(v, a, fbuf, line, t, c, lc, sm, so, ob);
@@ -325,7 +328,9 @@ struct XSmem {
 
 // Persistent: CTA b handles the row groups b, b + gridDim.x, ...; while one group is being transformed the next
 // one (psi rows and field rows) is requested into L2, so that its loads find the data there.
-template <int DT, int NX, int LINES, int MODE, int XS>
+// NEST: the real-space part is the nested split (PassXArgs::nest; its own instantiation, so that the default kernels
+// keep their register budget)
+template <int DT, int NX, int LINES, int MODE, int XS, bool NEST>
 __global__ void __launch_bounds__(LINES * (NX / 8), (LINES * (NX / 8) <= 256) ? 2 : 1)
 pass_x_kernel(const PassXArgs a) {
   typedef Plan<NX> P;
@@ -467,7 +472,7 @@ pass_x_kernel(const PassXArgs a) {
       __syncthreads();
       stage_fields<DT, NX, LINES, XS>(smem, a, first_point, grp * LINES, tid, &ffull, FBULK);
     };
-    if (MODE == MODE_MID || MODE == MODE_EPI) line_fft_inv<NX>(buf, twS, t, c, v, flip, fields_hook);
+    if (MODE == MODE_MID || mode_is_epi(MODE)) line_fft_inv<NX>(buf, twS, t, c, v, flip, fields_hook);
     TL_MARK(1);
 
     if (MODE != MODE_FWD) {
@@ -478,9 +483,9 @@ pass_x_kernel(const PassXArgs a) {
       // complete on the mbarrier every thread has just waited on
       if (!FBULK || a.V == nullptr || a.Om == nullptr || a.De == nullptr) __syncthreads();
       TL_MARK(2);
-      real_space<DT, NX, LINES, MODE>(v, a, smem, line, t, c, lc, sm, so, ob);
+      real_space<DT, NX, LINES, MODE, NEST>(v, a, smem, line, t, c, lc, sm, so, ob);
       TL_MARK(3);
-      if (MODE == MODE_EPI && (a.want_norm || a.want_obs)) {
+      if (mode_is_epi(MODE) && (a.want_norm || MODE == MODE_EPI_OBS)) {
         // norm partials of this row group, one slot per group: the sums do not depend on which CTA took the group,
         // so the reduction order (and every imaginary-time result) is the same from run to run.  Each lane summed
         // its own and the other component over its 8 points: sort into (up, down) first.
@@ -493,7 +498,7 @@ pass_x_kernel(const PassXArgs a) {
           sd += shfl_xor_d(sd, m);
         }
         if ((tid & 31) == 0) { red[0][tid >> 5] = su; red[1][tid >> 5] = sd; }
-        if (a.want_obs) {  // rho_up^2, rho_dn^2, rho_up rho_dn of the group (same sorting, same fixed order)
+        if (MODE == MODE_EPI_OBS) {  // rho_up^2, rho_dn^2, rho_up rho_dn of the group (same sorting, same fixed order)
           double quu = c ? ob.oo : ob.mm, qdd = c ? ob.mm : ob.oo, qud = ob.mo;
           ob.mm = ob.oo = ob.mo = 0.0;
 #pragma unroll
@@ -506,8 +511,8 @@ pass_x_kernel(const PassXArgs a) {
         }
       }
       __syncthreads();
-      if (MODE == MODE_EPI && (a.want_norm || a.want_obs) && tid == 0) {
-        const int nk = a.want_obs ? 5 : 2;
+      if (mode_is_epi(MODE) && (a.want_norm || MODE == MODE_EPI_OBS) && tid == 0) {
+        const int nk = MODE == MODE_EPI_OBS ? 5 : 2;
         for (int k = 0; k < nk; ++k) {
           double s0 = 0.0;
           for (int i = 0; i < NTHR / 32; ++i) s0 += red[k][i];
@@ -516,7 +521,7 @@ pass_x_kernel(const PassXArgs a) {
       }
     }
 
-    if (MODE != MODE_EPI) {
+    if (!mode_is_epi(MODE)) {
       fwd_stages<NX, 1>(buf, twS, t, c, v, flip, CtaSync());
       __syncthreads();  // the last exchange has been read by every warp: the line buffers are free
     }
@@ -526,7 +531,7 @@ pass_x_kernel(const PassXArgs a) {
       issue_loads(nxt_grp);
       if (tid == 0) nxt = sched_next(a.sched);  // consumed in the next iteration
     }
-    if (MODE == MODE_EPI) {
+    if (mode_is_epi(MODE)) {
 #pragma unroll
       for (int n = 0; n < 16; ++n) St::st(a.dst, (lbase + (size_t)(t + ((n + 8 * c) & 15) * T) * S) * 2 + c, v[n]);
     } else {
@@ -546,7 +551,7 @@ pass_x_kernel(const PassXArgs a) {
     grp = nxt_grp;
   }
   if (MODE == MODE_MID) TL_DUMP("xmid wait+stage|inv|fields|real|fwd|issue+last|ex+store", 7);
-  if (MODE == MODE_EPI) {
+  if (mode_is_epi(MODE)) {
     // imaginary time (a6): the CTA that finishes last turns the per-group norm partials into the rescale factors
     // of the next step (fixed summation order), so no separate kernel is needed
     __shared__ int last_s;
