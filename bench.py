@@ -6,7 +6,8 @@ two components, complex128, real time, dt = 2.5e-4), one JSON line on stdout.
 
 A "step" is one Strang step of the whole hot path (a6 in imaginary time).
   value      : grid-point-steps/s (P = nx*ny counted once, not per component) over all N replicas, state and
-               fields resident in HBM, CUDA events around ONE spgpe_step(K) call, max over ranks.
+               fields resident in HBM, CUDA events around ONE spgpe_step(K) call, max over ranks; --repeats (5)
+               such regions of exactly K steps are timed and the median one is reported with the MAD (`repeats`).
   e2e        : the same metric through the C ABI with HOST buffers: set_potential/raman/zeeman_host +
                set_psi_host (pinned) -> spgpe_step(K) -> get_psi_host, copies inside the timed region (the
                paper's usage: order parameter in, M steps, order parameter out).
@@ -42,17 +43,35 @@ WORKLOADS = {
 }
 
 
+KERNEL_SOURCES = ("common.cuh", "radix.cuh", "line_fft.cuh", "su2.cuh", "pass_x.cuh", "pass_y.cuh", "launch.cuh")
+
+
+def kernel_source_sha16() -> str:
+    """Hash of the sources the two pass kernels are compiled from (stamps profiles/r2_traffic.json)."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2010_15069_b200", "csrc", name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
 def read_traffic(workload: str, kernel: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full summary, or None."""
-    path = os.path.join(ROOT, "profiles", "r1_traffic.json")
+    """(bytes, source): dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full
+    summary profiles/r2_traffic.json.  The file names the commit and the hash of the kernel sources it was captured
+    from; when those sources have changed since, the number is stale and None is reported instead."""
+    path = os.path.join(ROOT, "profiles", "r2_traffic.json")
     try:
         with open(path) as f:
             d = json.load(f)
-        if d.get("workload") == workload:
-            return d["kernels"][kernel]["bytes_per_launch"]
-    except Exception:
-        pass
-    return None
+        if d.get("workload") != workload:
+            return None, f"profiles/r2_traffic.json holds {d.get('workload')}, not this workload"
+        if d.get("kernel_source_sha16") != kernel_source_sha16():
+            return None, "profiles/r2_traffic.json is stale (kernel sources changed since the capture)"
+        return d["kernels"][kernel]["bytes_per_launch"], (f"ncu --set full at commit {d.get('captured_at_commit')}, "
+                                                           "profiles/r2_ncu_full.md")
+    except Exception as e:
+        return None, f"no traffic record ({type(e).__name__})"
 
 
 def read_peaks():
@@ -118,12 +137,15 @@ class ClockSampler:
                 "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
-def oracle_sample(w_cfg: int, dtype: str, budget_s: float, steps: int):
+def oracle_sample(w_cfg: int, dtype: str, budget_s: float, steps: int, threads: int = 0):
     """Times the oracle on a proxy grid of the same recipe, chosen so that `steps` steps fit the budget.
-    Returns (grid-point-steps/s, threads, description, seconds per step)."""
+    threads = 0: every host core (OpenMP), else that many.  Returns (grid-point-steps/s, threads, description,
+    seconds per step)."""
     import oracle as orc
     import workloads as wl
-    threads = orc.max_threads()
+    all_threads = orc.max_threads()
+    orc.set_threads(threads or all_threads)
+    threads = threads or all_threads
     full = wl.CONFIGS[w_cfg]["n"]
     n, sec = 64, None
     while True:
@@ -136,12 +158,14 @@ def oracle_sample(w_cfg: int, dtype: str, budget_s: float, steps: int):
         if n >= full or 4.2 * sec * steps > budget_s:  # the next size costs ~4.2x
             break
         n *= 2
-    steps = int(min(200, max(steps, 12.0 / max(sec, 1e-3))))  # about 12 s of CPU work
+    steps = int(min(200, max(steps, 0.5 * budget_s / max(sec, 1e-3))))  # about half the budget of CPU work
     t0 = time.perf_counter()
     orc.step(w.psi0, w.V, w.Omega, w.delta, p, steps, dt, imag)
     sec = (time.perf_counter() - t0) / steps
-    what = (f"{steps} oracle steps (fp64, own radix-2 FFT, OpenMP) of config {w_cfg}'s recipe on a {n}x{n} "
-            f"grid (full size {full}x{full}), {'imaginary' if imag else 'real'} time")
+    orc.set_threads(all_threads)
+    what = (f"{steps} oracle steps (fp64, own radix-2 FFT, {threads} OpenMP thread{'s' if threads > 1 else ''}) of "
+            f"config {w_cfg}'s recipe on a {n}x{n} grid (full size {full}x{full}), "
+            f"{'imaginary' if imag else 'real'} time")
     return n * n / sec, threads, what, sec
 
 
@@ -239,6 +263,8 @@ def run_ours(args, wname):
         torch.cuda.synchronize()
 
     def timed_region(fn):
+        """One region of exactly K steps: barrier + synchronize, CUDA events on the handle's stream, barrier +
+        synchronize; returns the max over ranks in ms."""
         barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         with torch.cuda.stream(stream):
@@ -254,8 +280,12 @@ def run_ours(args, wname):
     sp.spgpe_synchronize(h)
     sampler.start()
     l0 = sp.spgpe_launch_count(h)
-    ms = timed_region(lambda: sp.spgpe_step(h, K, dt, imag))
-    launches = sp.spgpe_launch_count(h) - l0
+    # the paper's statistic: REPEATS regions of exactly K steps each, median and
+    # median absolute deviation; `value` and `ms_per_step` are the median region's
+    region_ms = [timed_region(lambda: sp.spgpe_step(h, K, dt, imag)) for _ in range(args.repeats)]
+    launches = (sp.spgpe_launch_count(h) - l0) // args.repeats
+    ms = float(np.median(region_ms))
+    mad_ms = float(np.median(np.abs(np.array(region_ms) - ms)))
     # ---- per-launch durations of the two pass kernels (second region of K steps) -----------------------
     sp.spgpe_profile(h, True)
     sp.spgpe_step(h, K, dt, imag)
@@ -298,6 +328,7 @@ def run_ours(args, wname):
         step_bytes = (bytes_pt[0] + bytes_pt[1]) * P
         flops_pt = 20.0 * np.log2(float(P)) + 360.0
         dfma_tf = sp.spgpe_probe_dfma(stream.cuda_stream)
+        traffic, traffic_src = read_traffic(w.name, ["pass_x_kernel", "pass_y_kernel"][dom])
         line = {
             "metric": METRIC, "value": world * P * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
             "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -307,12 +338,14 @@ def run_ours(args, wname):
                        "l2": f"state {psi_bytes >> 20} MiB + fields {(nfields * P * rsz) >> 20} MiB per replica; "
                              + ("larger than the 126 MB L2, no flush" if psi_bytes > 126e6 else
                                 "fits L2: the HBM roofline is not the binding bound")},
+            "repeats": {"regions": args.repeats, "steps_per_region": K, "ms_per_step_median": ms / K,
+                        "ms_per_step_mad": mad_ms / K, "ms_per_step_all": [r / K for r in region_ms]},
             "steps_per_s": world * K / (ms * 1e-3),
             "step_hbm_gbs": step_bytes / (ms / K * 1e-3) / 1e9,
             "step_roofline_frac": step_bytes / (ms / K * 1e-3) / 1e9 / peak,
             "roofline": {"bound": "hbm", "kernel": ["pass_x_kernel (row pass)", "pass_y_kernel (column pass)"][dom],
                          "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": read_traffic(w.name, ["pass_x_kernel", "pass_y_kernel"][dom]),
+                         "traffic": traffic, "traffic_source": traffic_src,
                          "algorithmic_bytes": bytes_pt[dom] * P, "peak_source": peak_src,
                          "avg_launch_us": {"row_pass": 1e3 * avg[0], "column_pass": 1e3 * avg[1]},
                          "launches_timed": kcnt, "bytes_per_point": bytes_pt},
@@ -328,9 +361,12 @@ def run_ours(args, wname):
             "gpu_launches": int(launches), "clocks": clocks, "finite": finite, "norms": list(map(float, norms)),
         }
         if world == 1 and not args.no_cpu:
-            v, cores, what, sec = oracle_sample(spec["cfg"], spec["dtype"], budget_s=25.0, steps=3)
+            v, cores, what, sec = oracle_sample(spec["cfg"], spec["dtype"], budget_s=20.0, steps=3)
+            v1, _, what1, sec1 = oracle_sample(spec["cfg"], spec["dtype"], budget_s=10.0, steps=3, threads=1)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what,
-                                    "s_per_step": sec}
+                                    "s_per_step": sec,
+                                    "single_thread": {"value": v1, "unit": UNIT, "cores": 1, "sample": what1,
+                                                      "s_per_step": sec1}}
         print(json.dumps(line), flush=True)
     sp.spgpe_destroy(h)
     if world > 1:
@@ -342,12 +378,14 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--repeats", type=int, default=5, help="timed regions of --steps steps each (median reported)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="4", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
+    args.repeats = max(1, args.repeats)
     if args.impl == "reference":
         run_reference(args, args.workload)
     else:
