@@ -30,6 +30,8 @@ struct spgpe_ctx {
   void *Vbuf, *Ombuf, *Debuf;  // owned storage
   const void *V, *Om, *De;     // NULL = zero field
   double2 *tw_x, *tw_y;
+  float4 *tw_x32, *tw_y32, *exk32, *eyk32;  // two-float twiddles and phase tables of the fp32 kernels (complex64 storage)
+  bool f32_ok;           // complex64 storage, unsplit axes: plain steps run on the fp32 kernels (pass32.cuh)
   double *Kx, *Ky;       // kinetic tables in stored order: Kx[2][nx], Ky[ny]
   double* kxv;           // k_x in stored order [nx] (observables)
   double* kpartial;      // [KPARTIAL_ROWS][6] k-space sums of the observed column pass
@@ -43,7 +45,7 @@ struct spgpe_ctx {
   int tab_imag;
   bool tab_valid;
   double *partial, *scale, *target, *dout;
-  CUtensorMap tmap_psi, tmap_scratch, tmap_psi_db, tmap_psi_duo;  // column-pass tensor maps of psi / the energy scratch buffer
+  CUtensorMap tmap_psi, tmap_scratch, tmap_psi_db, tmap_psi_duo, tmap_psi32;  // column-pass tensor maps of psi / the energy scratch buffer
   int* sched;    // [4] work counters of the persistent kernels: row pass [0..1], column pass [2..3]
   double2 *wcx, *wcy;         // split axes: join twiddles
   int *fpx, *fpy;             // split axes: true frequency of a sub-transform position
@@ -155,6 +157,20 @@ static int env_int(const char* name) {
 
 static cudaError_t dispatch_x_raw(spgpe_ctx* h, int mode, const PassXArgs& a) {
   const int nl = h->ny * h->sx;  // lines
+  // complex64 storage: the plain passes run on the fp32 kernels; the nested split, the observed closing pass, an
+  // annealed opening pass and the transform-only mode stay on the fp64-arithmetic kernels (same layout)
+  if (h->f32_ok && !a.nest && (mode == MODE_PRO || mode == MODE_MID || mode == MODE_EPI) &&
+      !(mode == MODE_PRO && a.anneal_event > 0)) {
+    switch (h->mx) {
+      case 64: return launch_row32_64(mode, a, nl, h->stream, h->env, &h->xgrid);
+      case 128: return launch_row32_128(mode, a, nl, h->stream, h->env, &h->xgrid);
+      case 256: return launch_row32_256(mode, a, nl, h->stream, h->env, &h->xgrid);
+      case 512: return launch_row32_512(mode, a, nl, h->stream, h->env, &h->xgrid);
+      case 1024: return launch_row32_1024(mode, a, nl, h->stream, h->env, &h->xgrid);
+      case 2048: return launch_row32_2048(mode, a, nl, h->stream, h->env, &h->xgrid);
+      default: return launch_row32_4096(mode, a, nl, h->stream, h->env, &h->xgrid);
+    }
+  }
   switch (h->mx) {
     case 64: return launch_pass_x_64(h->dt, mode, a, nl, h->stream, h->env, &h->xgrid);
     case 128: return launch_pass_x_128(h->dt, mode, a, nl, h->stream, h->env, &h->xgrid);
@@ -166,6 +182,17 @@ static cudaError_t dispatch_x_raw(spgpe_ctx* h, int mode, const PassXArgs& a) {
   }
 }
 static cudaError_t dispatch_y_raw(spgpe_ctx* h, int ymode, const PassYArgs& a) {
+  if (h->f32_ok && ymode == YMODE_STEP) {
+    switch (h->my) {
+      case 64: return launch_col32_64(a, h->stream, h->env, &h->ygrid);
+      case 128: return launch_col32_128(a, h->stream, h->env, &h->ygrid);
+      case 256: return launch_col32_256(a, h->stream, h->env, &h->ygrid);
+      case 512: return launch_col32_512(a, h->stream, h->env, &h->ygrid);
+      case 1024: return launch_col32_1024(a, h->stream, h->env, &h->ygrid);
+      case 2048: return launch_col32_2048(a, h->stream, h->env, &h->ygrid);
+      default: return launch_col32_4096(a, h->stream, h->env, &h->ygrid);
+    }
+  }
   switch (h->my) {
     case 64: return launch_pass_y_64(h->dt, ymode, a, h->stream, h->env, &h->ygrid);
     case 128: return launch_pass_y_128(h->dt, ymode, a, h->stream, h->env, &h->ygrid);
@@ -280,6 +307,11 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
   alloc((void**)&h->kpartial, sizeof(double) * 6 * KPARTIAL_ROWS);
   alloc((void**)&h->exk, sizeof(double2) * 2 * nx);
   alloc((void**)&h->eyk, sizeof(double2) * ny);
+  alloc((void**)&h->exk32, sizeof(float4) * 2 * nx);
+  alloc((void**)&h->eyk32, sizeof(float4) * ny);
+  alloc((void**)&h->tw_x32, sizeof(float4) * (twx > 0 ? twx : 1));
+  alloc((void**)&h->tw_y32, sizeof(float4) * (twy > 0 ? twy : 1));
+  h->f32_ok = h->dt == SPGPE_C64 && h->sx == 1 && h->sy == 1 && !env_int("SPGPE_DEBUG_NO_F32");
   alloc((void**)&h->partial, sizeof(double) * h->partial_cap);
   alloc((void**)&h->scale, sizeof(double) * 2);
   alloc((void**)&h->target, sizeof(double) * 2);
@@ -295,6 +327,15 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
     if (e == cudaSuccess) {
       plan_fill_twiddles(h->my, tw.data());
       e = cudaMemcpy(h->tw_y, tw.data(), sizeof(double2) * twy, cudaMemcpyHostToDevice);
+    }
+    std::vector<float4> tw32(twx > twy ? twx : twy);
+    if (e == cudaSuccess) {
+      plan_fill_twiddles32(h->mx, tw32.data());
+      e = cudaMemcpy(h->tw_x32, tw32.data(), sizeof(float4) * twx, cudaMemcpyHostToDevice);
+    }
+    if (e == cudaSuccess) {
+      plan_fill_twiddles32(h->my, tw32.data());
+      e = cudaMemcpy(h->tw_y32, tw32.data(), sizeof(float4) * twy, cudaMemcpyHostToDevice);
     }
   }
   if (e == cudaSuccess) {
@@ -324,6 +365,7 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
     if (e == cudaSuccess) e = cudaMemcpy(*dwc, wc.data(), sizeof(double2) * m, cudaMemcpyHostToDevice);
   }
   if (e == cudaSuccess) e = make_col_tmap(h, h->psi, plan_lines_y(h->my), &h->tmap_psi);
+  if (e == cudaSuccess && h->f32_ok) e = make_col_tmap(h, h->psi, plan_lines_y32(h->my), &h->tmap_psi32);
   if (e == cudaSuccess && plan_lines_ydb(h->my) > 0) e = make_col_tmap(h, h->psi, plan_lines_ydb(h->my), &h->tmap_psi_db);
   if (e == cudaSuccess && plan_has_duo(h->my) && h->dt == SPGPE_C128) e = make_col_tmap(h, h->psi, 1, &h->tmap_psi_duo, h->my / 16);
   if (e != cudaSuccess) {
@@ -339,7 +381,7 @@ extern "C" int spgpe_destroy(spgpe_handle h) {
   ON_DEVICE(h);
   cudaStreamSynchronize(h->stream);
   void* ptrs[] = {h->psi, h->scratch, h->Vbuf, h->Ombuf, h->Debuf, h->tw_x, h->tw_y, h->Kx, h->Ky, h->kxv, h->kpartial,
-                  h->exk, h->eyk, h->partial, h->scale, h->target, h->dout, h->fmax, h->sched, h->wcx, h->wcy, h->fpx, h->fpy};
+                  h->exk, h->eyk, h->exk32, h->eyk32, h->tw_x32, h->tw_y32, h->partial, h->scale, h->target, h->dout, h->fmax, h->sched, h->wcx, h->wcy, h->fpx, h->fpy};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   if (h->prof_ev) {
@@ -431,7 +473,7 @@ extern "C" int spgpe_set_norm_targets(spgpe_handle h, double n_up, double n_dn) 
 static int ensure_tables(spgpe_handle h, double dt, int imag) {
   if (h->tab_valid && h->tab_dt == dt && h->tab_imag == imag) return SPGPE_OK;
   h->launches++;
-  CK(aux_phase_tables(h->Kx, h->Ky, h->nx, h->ny, dt, imag, h->exk, h->eyk, h->stream));
+  CK(aux_phase_tables(h->Kx, h->Ky, h->nx, h->ny, dt, imag, h->exk, h->eyk, h->exk32, h->eyk32, h->stream));
   h->tab_dt = dt; h->tab_imag = imag; h->tab_valid = true;
   return SPGPE_OK;
 }
@@ -476,7 +518,7 @@ static int step_impl(spgpe_handle h, int n, double dt, int imag, bool obs) {
   PassXArgs xa;
   memset(&xa, 0, sizeof(xa));
   xa.src = h->psi; xa.dst = h->psi; xa.V = h->V; xa.Om = h->Om; xa.De = h->De;
-  xa.tw = h->tw_x; xa.scale = nullptr; xa.partial = h->partial;
+  xa.tw = h->tw_x; xa.tw32 = h->tw_x32; xa.scale = nullptr; xa.partial = h->partial;
   xa.tau = 0.5 * dt; xa.hc = h->hc; xa.imag = imag; xa.want_norm = imag; xa.ny = h->ny * h->sx; xa.xs = h->sx;
   xa.fmax = h->fmax; xa.sched = h->sched; xa.dbg = h->env.xdbg;
   xa.target = h->target; xa.scale_out = h->scale; xa.cell = (h->Lx / h->nx) * (h->Ly / h->ny); xa.norm_mode = h->p.norm_mode;
@@ -485,6 +527,7 @@ static int step_impl(spgpe_handle h, int n, double dt, int imag, bool obs) {
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
   ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx * h->sy;
+  ya.tw32 = h->tw_y32; ya.eyk32 = h->eyk32; ya.exk32 = h->exk32; ya.tmap32 = h->tmap_psi32;
   // the k_x phase rides on the column pass unless a split axis sends the k-space phases to the join kernel
   ya.exk = (h->sx == 1 && h->sy == 1) ? h->exk : nullptr; ya.sched = h->sched + 2; ya.tmap = h->tmap_psi; ya.tmap_db = h->tmap_psi_db; ya.tmap_duo = h->tmap_psi_duo;
   // the observed column pass (last step only): k-space sums per CTA into kpartial

@@ -7,7 +7,7 @@ namespace spgpe {
 // ---- k-space phase tables (Eq. 5, R-1..R-3) ---------------------------------------
 // exk[c][pos] = exp(-i Kx_c dt) (imag: exp(-Kx_c dt)); eyk[pos] = exp(-i Ky dt) / (nx ny) (imag: exp(-Ky dt)/(nx ny))
 __global__ void phase_tables_kernel(const double* __restrict__ Kx, const double* __restrict__ Ky, int nx, int ny,
-                                    double dt, int imag, double2* exk, double2* eyk) {
+                                    double dt, int imag, double2* exk, double2* eyk, float4* exk32, float4* eyk32) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int total = 2 * nx + ny;
   if (i >= total) return;
@@ -22,14 +22,17 @@ __global__ void phase_tables_kernel(const double* __restrict__ Kx, const double*
     sincos(K * dt, &sn, &cn);
     r = make_double2(s * cn, -s * sn);
   }
-  if (is_y) eyk[i - 2 * nx] = r;
-  else exk[i] = r;
+  // the same factors as two-float values for the fp32 kernels (fft32.cuh)
+  const float hr = (float)r.x, hi = (float)r.y;
+  const float4 r32 = make_float4(hr, hi, (float)(r.x - (double)hr), (float)(r.y - (double)hi));
+  if (is_y) { eyk[i - 2 * nx] = r; eyk32[i - 2 * nx] = r32; }
+  else { exk[i] = r; exk32[i] = r32; }
 }
 
 cudaError_t aux_phase_tables(const double* Kx, const double* Ky, int nx, int ny, double dt, int imag,
-                             double2* exk, double2* eyk, cudaStream_t s) {
+                             double2* exk, double2* eyk, float4* exk32, float4* eyk32, cudaStream_t s) {
   const int total = 2 * nx + ny;
-  phase_tables_kernel<<<(total + 255) / 256, 256, 0, s>>>(Kx, Ky, nx, ny, dt, imag, exk, eyk);
+  phase_tables_kernel<<<(total + 255) / 256, 256, 0, s>>>(Kx, Ky, nx, ny, dt, imag, exk, eyk, exk32, eyk32);
   return cudaGetLastError();
 }
 

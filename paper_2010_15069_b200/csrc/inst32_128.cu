@@ -1,0 +1,5 @@
+// inst32_128.cu -- fp32 row/column pass kernels for line length 128 (see launch32.cuh)
+#include "launch32.cuh"
+namespace spgpe {
+SPGPE_DEFINE_LAUNCHERS32(128)
+}

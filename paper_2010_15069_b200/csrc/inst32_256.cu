@@ -1,0 +1,5 @@
+// inst32_256.cu -- fp32 row/column pass kernels for line length 256 (see launch32.cuh)
+#include "launch32.cuh"
+namespace spgpe {
+SPGPE_DEFINE_LAUNCHERS32(256)
+}

@@ -21,6 +21,19 @@ SPGPE_DECL(1024)
 SPGPE_DECL(2048)
 SPGPE_DECL(4096)
 #undef SPGPE_DECL
+// fp32 kernels of the complex64 path (inst32_<N>.cu, pass32.cuh)
+#define SPGPE_DECL32(N_)                                                                                      \
+  cudaError_t launch_row32_##N_(int mode, const PassXArgs& a, int ny, cudaStream_t s, const LaunchEnv& env,  \
+                                int* grid);                                                                    \
+  cudaError_t launch_col32_##N_(const PassYArgs& a, cudaStream_t s, const LaunchEnv& env, int* grid);
+SPGPE_DECL32(64)
+SPGPE_DECL32(128)
+SPGPE_DECL32(256)
+SPGPE_DECL32(512)
+SPGPE_DECL32(1024)
+SPGPE_DECL32(2048)
+SPGPE_DECL32(4096)
+#undef SPGPE_DECL32
 
 // join of the two interleaved sub-transforms of an axis longer than 4096 (split.cu)
 struct SplitArgs {
@@ -45,11 +58,14 @@ int plan_lines_ydb(int n);                      // columns per tile of the doubl
 bool plan_has_duo(int n);                       // a two-group column pass exists for length n (complex128)
 int plan_lines_x(int n);                        // rows per CTA of the row pass of length n
 int plan_lines_y(int n);                        // columns per CTA of the column pass of length n
+int plan_lines_x32(int n);                      // rows / columns per CTA of the fp32 kernels (pass32.cuh)
+int plan_lines_y32(int n);
+void plan_fill_twiddles32(int n, float4* host); // the twiddles of plan_fill_twiddles as two-float values
 int plan_freq_of_pos(int n, int pos);           // signed-less frequency index f in [0, n) stored at position pos
 
 // small kernels (aux.cu); all enqueue on s and return cudaGetLastError()
 cudaError_t aux_phase_tables(const double* Kx, const double* Ky, int nx, int ny, double dt, int imag,
-                             double2* exk, double2* eyk, cudaStream_t s);
+                             double2* exk, double2* eyk, float4* exk32, float4* eyk32, cudaStream_t s);
 // partial[nblk][ncol] -> out[col] = factor * sum_blk partial[blk][col]   (fixed summation order)
 cudaError_t aux_sum_partials(const double* partial, int nblk, int ncol, double factor, double* out,
                              cudaStream_t s);

@@ -30,6 +30,7 @@ struct PassXArgs {
   const void* Om;
   const void* De;
   const double2* tw;     // twiddles of NX
+  const float4* tw32;    // the same twiddles as two-float values (hi.re, hi.im, lo.re, lo.im): fp32 kernels, pass32.cuh
   const double* scale;   // [2] per-component factor applied at load (MODE_PRO, imaginary time) or NULL
   double* partial;       // [ny / LINES][pstride] sums of every row group (MODE_EPI with want_norm, MODE_EPI_OBS)
   double tau;            // half-step size dt/2

@@ -25,6 +25,9 @@ enum { YMODE_STEP = 0, YMODE_ENERGY = 1, YMODE_FWDONLY = 2, YMODE_INVONLY = 3, Y
 struct PassYArgs {
   void* psi;            // [NY][nx][2]
   const double2* tw;    // twiddles of NY
+  const float4* tw32;   // two-float twiddles, k_y phases [NY] and k_x phases [2][nx] of the fp32 kernels (pass32.cuh)
+  const float4* eyk32;
+  const float4* exk32;
   const double2* eyk;   // [NY] k_y phase in stored order (YMODE_STEP)
   const double2* exk;   // [2][nx] k_x phase in the row pass's stored order (YMODE_STEP), or NULL (none applied here)
   const double* Kx;     // [2][nx] (k_x +- k_L)^2/2 in the row pass's stored order (YMODE_ENERGY)
@@ -37,6 +40,7 @@ struct PassYArgs {
   CUtensorMap tmap;
   CUtensorMap tmap_db;  // the same tensor with the box of the double-buffered kernel (pass_y_db_kernel)
   CUtensorMap tmap_duo; // the same tensor, box = [NY/16 rows][one column] (pass_y_duo_kernel)
+  CUtensorMap tmap32;   // the same tensor with the tile of col32_kernel (pass32.cuh)
 };
 
 template <int NY, int LINES>

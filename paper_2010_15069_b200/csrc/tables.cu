@@ -4,6 +4,7 @@
 
 #include "internal.h"
 #include "launch.cuh"
+#include "pass32.cuh"
 
 namespace spgpe {
 
@@ -36,6 +37,28 @@ int plan_lines_x(int n) {
     default: return Lines<4096>::X;
   }
 }
+int plan_lines_x32(int n) {
+  switch (n) {
+    case 64: return Lines32<64>::X;
+    case 128: return Lines32<128>::X;
+    case 256: return Lines32<256>::X;
+    case 512: return Lines32<512>::X;
+    case 1024: return Lines32<1024>::X;
+    case 2048: return Lines32<2048>::X;
+    default: return Lines32<4096>::X;
+  }
+}
+int plan_lines_y32(int n) {
+  switch (n) {
+    case 64: return Lines32<64>::Y;
+    case 128: return Lines32<128>::Y;
+    case 256: return Lines32<256>::Y;
+    case 512: return Lines32<512>::Y;
+    case 1024: return Lines32<1024>::Y;
+    case 2048: return Lines32<2048>::Y;
+    default: return Lines32<4096>::Y;
+  }
+}
 int plan_lines_ydb(int n) { return n == 2048 ? Lines<2048>::YDB : (n == 1024 ? Lines<1024>::YDB : 0); }
 
 bool plan_has_duo(int n) { return n == 2048 ? Lines<2048>::DUO : (n == 1024 ? Lines<1024>::DUO : false); }
@@ -62,6 +85,18 @@ void plan_fill_twiddles(int n, double2* host) {
       }
     off += 15 * M;
   }
+}
+
+// hi = fp32 rounding of the fp64 twiddle, lo = fp32 rounding of the remainder (fft32.cuh)
+void plan_fill_twiddles32(int n, float4* host) {
+  const int total = plan_tw_total(n);
+  double2* tmp = new double2[total > 0 ? total : 1];
+  plan_fill_twiddles(n, tmp);
+  for (int i = 0; i < total; ++i) {
+    const float hr = (float)tmp[i].x, hi = (float)tmp[i].y;
+    host[i] = make_float4(hr, hi, (float)(tmp[i].x - (double)hr), (float)(tmp[i].y - (double)hi));
+  }
+  delete[] tmp;
 }
 
 // Frequency index held at stored position pos = (t + g*T) + (n/RL) * s (T = n/16 threads per component, thread t,
