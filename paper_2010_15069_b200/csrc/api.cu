@@ -31,7 +31,8 @@ struct spgpe_ctx {
   const void *V, *Om, *De;     // NULL = zero field
   double2 *tw_x, *tw_y;
   float4 *tw_x32, *tw_y32, *exk32, *eyk32;  // two-float twiddles and phase tables of the fp32 kernels (complex64 storage)
-  bool f32_ok;           // complex64 storage, unsplit axes: plain steps run on the fp32 kernels (pass32.cuh)
+  int f32_dbg;           // SPGPE_DEBUG_NO_F32: 1 no fp32 kernels, 2 fp32 column pass only, 3 fp32 row pass only
+  bool f32_ok;           // complex64 storage: the passes of plain steps run on the fp32 kernels (pass32.cuh)
   double *Kx, *Ky;       // kinetic tables in stored order: Kx[2][nx], Ky[ny]
   double* kxv;           // k_x in stored order [nx] (observables)
   double* kpartial;      // [KPARTIAL_ROWS][6] k-space sums of the observed column pass
@@ -159,8 +160,8 @@ static cudaError_t dispatch_x_raw(spgpe_ctx* h, int mode, const PassXArgs& a) {
   const int nl = h->ny * h->sx;  // lines
   // complex64 storage: the plain passes run on the fp32 kernels; the nested split, the observed closing pass, an
   // annealed opening pass and the transform-only mode stay on the fp64-arithmetic kernels (same layout)
-  if (h->f32_ok && !a.nest && (mode == MODE_PRO || mode == MODE_MID || mode == MODE_EPI) &&
-      !(mode == MODE_PRO && a.anneal_event > 0)) {
+  if (h->f32_ok && h->f32_dbg != 2 && a.tw32 != nullptr && !a.nest && (mode == MODE_PRO || mode == MODE_MID || mode == MODE_EPI) &&
+      !(mode == MODE_PRO && a.anneal_event > 0) && (a.xs == 1 || h->mx >= 512)) {
     switch (h->mx) {
       case 64: return launch_row32_64(mode, a, nl, h->stream, h->env, &h->xgrid);
       case 128: return launch_row32_128(mode, a, nl, h->stream, h->env, &h->xgrid);
@@ -182,15 +183,15 @@ static cudaError_t dispatch_x_raw(spgpe_ctx* h, int mode, const PassXArgs& a) {
   }
 }
 static cudaError_t dispatch_y_raw(spgpe_ctx* h, int ymode, const PassYArgs& a) {
-  if (h->f32_ok && ymode == YMODE_STEP) {
+  if (h->f32_ok && h->f32_dbg != 3 && a.tw32 != nullptr && (ymode == YMODE_STEP || ymode == YMODE_FWDONLY || ymode == YMODE_INVONLY)) {
     switch (h->my) {
-      case 64: return launch_col32_64(a, h->stream, h->env, &h->ygrid);
-      case 128: return launch_col32_128(a, h->stream, h->env, &h->ygrid);
-      case 256: return launch_col32_256(a, h->stream, h->env, &h->ygrid);
-      case 512: return launch_col32_512(a, h->stream, h->env, &h->ygrid);
-      case 1024: return launch_col32_1024(a, h->stream, h->env, &h->ygrid);
-      case 2048: return launch_col32_2048(a, h->stream, h->env, &h->ygrid);
-      default: return launch_col32_4096(a, h->stream, h->env, &h->ygrid);
+      case 64: return launch_col32_64(ymode, a, h->stream, h->env, &h->ygrid);
+      case 128: return launch_col32_128(ymode, a, h->stream, h->env, &h->ygrid);
+      case 256: return launch_col32_256(ymode, a, h->stream, h->env, &h->ygrid);
+      case 512: return launch_col32_512(ymode, a, h->stream, h->env, &h->ygrid);
+      case 1024: return launch_col32_1024(ymode, a, h->stream, h->env, &h->ygrid);
+      case 2048: return launch_col32_2048(ymode, a, h->stream, h->env, &h->ygrid);
+      default: return launch_col32_4096(ymode, a, h->stream, h->env, &h->ygrid);
     }
   }
   switch (h->my) {
@@ -311,7 +312,8 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
   alloc((void**)&h->eyk32, sizeof(float4) * ny);
   alloc((void**)&h->tw_x32, sizeof(float4) * (twx > 0 ? twx : 1));
   alloc((void**)&h->tw_y32, sizeof(float4) * (twy > 0 ? twy : 1));
-  h->f32_ok = h->dt == SPGPE_C64 && h->sx == 1 && h->sy == 1 && !env_int("SPGPE_DEBUG_NO_F32");
+  h->f32_dbg = env_int("SPGPE_DEBUG_NO_F32");
+  h->f32_ok = h->dt == SPGPE_C64 && h->f32_dbg != 1;
   alloc((void**)&h->partial, sizeof(double) * h->partial_cap);
   alloc((void**)&h->scale, sizeof(double) * 2);
   alloc((void**)&h->target, sizeof(double) * 2);
@@ -527,7 +529,8 @@ static int step_impl(spgpe_handle h, int n, double dt, int imag, bool obs) {
   PassYArgs ya;
   memset(&ya, 0, sizeof(ya));
   ya.psi = h->psi; ya.tw = h->tw_y; ya.eyk = h->eyk; ya.nx = h->nx * h->sy;
-  ya.tw32 = h->tw_y32; ya.eyk32 = h->eyk32; ya.exk32 = h->exk32; ya.tmap32 = h->tmap_psi32;
+  ya.tw32 = h->tw_y32; ya.eyk32 = h->eyk32; ya.tmap32 = h->tmap_psi32;
+  ya.exk32 = (h->sx == 1 && h->sy == 1) ? h->exk32 : nullptr;
   // the k_x phase rides on the column pass unless a split axis sends the k-space phases to the join kernel
   ya.exk = (h->sx == 1 && h->sy == 1) ? h->exk : nullptr; ya.sched = h->sched + 2; ya.tmap = h->tmap_psi; ya.tmap_db = h->tmap_psi_db; ya.tmap_duo = h->tmap_psi_duo;
   // the observed column pass (last step only): k-space sums per CTA into kpartial

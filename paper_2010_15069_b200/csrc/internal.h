@@ -25,7 +25,7 @@ SPGPE_DECL(4096)
 #define SPGPE_DECL32(N_)                                                                                      \
   cudaError_t launch_row32_##N_(int mode, const PassXArgs& a, int ny, cudaStream_t s, const LaunchEnv& env,  \
                                 int* grid);                                                                    \
-  cudaError_t launch_col32_##N_(const PassYArgs& a, cudaStream_t s, const LaunchEnv& env, int* grid);
+  cudaError_t launch_col32_##N_(int ymode, const PassYArgs& a, cudaStream_t s, const LaunchEnv& env, int* grid);
 SPGPE_DECL32(64)
 SPGPE_DECL32(128)
 SPGPE_DECL32(256)

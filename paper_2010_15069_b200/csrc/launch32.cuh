@@ -5,10 +5,10 @@
 
 namespace spgpe {
 
-template <int N, int MODE>
-cudaError_t launch_row32(const PassXArgs& a, int ny, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
-  constexpr int L = Lines32<N>::X;
-  auto k = row32_kernel<N, L, MODE>;
+template <int N, int MODE, int XS>
+cudaError_t launch_row32_xs(const PassXArgs& a, int ny, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
+  constexpr int L = (XS == 2) ? 2 : Lines32<N>::X;
+  auto k = row32_kernel<N, L, MODE, XS>;
   constexpr size_t smem = Smem32<N, L>::BYTES_X;
   static int cache[SPGPE_MAX_DEVICES] = {};
   int resident = 0;
@@ -20,10 +20,19 @@ cudaError_t launch_row32(const PassXArgs& a, int ny, cudaStream_t s, const Launc
   return launch_pdl(k, grid, L * (N / 16), smem, s, a);
 }
 
-template <int N>
+// a split x axis (xs = 2) is handled by the fp32 kernels from sub-line length 512 up (full warps per line pair)
+template <int N, int MODE>
+cudaError_t launch_row32(const PassXArgs& a, int ny, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
+  if constexpr (N >= 512) {
+    if (a.xs == 2) return launch_row32_xs<N, MODE, 2>(a, ny, s, env, grid_out);
+  }
+  return launch_row32_xs<N, MODE, 1>(a, ny, s, env, grid_out);
+}
+
+template <int N, int YMODE>
 cudaError_t launch_col32(const PassYArgs& a, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
   constexpr int L = Lines32<N>::Y;
-  auto k = col32_kernel<N, L>;
+  auto k = col32_kernel<N, L, YMODE>;
   constexpr size_t smem = Smem32<N, L>::BYTES_Y;
   static int cache[SPGPE_MAX_DEVICES] = {};
   int resident = 0;
@@ -44,8 +53,12 @@ cudaError_t launch_col32(const PassYArgs& a, cudaStream_t s, const LaunchEnv& en
       default: return launch_row32<N_, MODE_EPI>(a, ny, s, env, g);                                                \
     }                                                                                                              \
   }                                                                                                                \
-  cudaError_t launch_col32_##N_(const PassYArgs& a, cudaStream_t s, const LaunchEnv& env, int* g) {              \
-    return launch_col32<N_>(a, s, env, g);                                                                         \
+  cudaError_t launch_col32_##N_(int ymode, const PassYArgs& a, cudaStream_t s, const LaunchEnv& env, int* g) {   \
+    switch (ymode) {                                                                                               \
+      case YMODE_STEP: return launch_col32<N_, YMODE_STEP>(a, s, env, g);                                          \
+      case YMODE_FWDONLY: return launch_col32<N_, YMODE_FWDONLY>(a, s, env, g);                                    \
+      default: return launch_col32<N_, YMODE_INVONLY>(a, s, env, g);                                               \
+    }                                                                                                              \
   }
 
 }  // namespace spgpe

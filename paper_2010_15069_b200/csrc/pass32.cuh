@@ -37,11 +37,13 @@ struct Smem32 {
 };
 
 // ---- real-space part on one thread's 16 points (both components in the thread) ----------------------------------
-template <int NX, int LINES, int MODE, int TIER, bool BZ0>
+// XS = 2: the LINES = 2 lines of the CTA are the even and the odd points of ONE row (split x axis, split.cu): point x of
+// line `line` is point 2 x + line of the row, in the staged row as well as in the staged fields.
+template <int NX, int LINES, int MODE, int TIER, bool BZ0, int XS>
 __device__ __forceinline__ void real_space32_tier(cf* u, cf* d, const PassXArgs& a, const float* fbuf, int line, int t,
                                                   const LaneCoef& lc, double& su, double& sd) {
-  constexpr int T = NX / 16;
-  const float* fV = fbuf + line * NX + t;
+  constexpr int T = (XS == 1) ? NX / 16 : 2 * (NX / 16);  // distance of a thread's consecutive points in the field rows
+  const float* fV = fbuf + (XS == 1 ? line * NX + t : 2 * t + line);
   const float* fO = fV + LINES * NX;
   const float* fD = fO + LINES * NX;
   const double tau = a.tau, tau2 = a.tau * a.tau;
@@ -82,7 +84,7 @@ __device__ __forceinline__ void real_space32_tier(cf* u, cf* d, const PassXArgs&
   }
 }
 
-template <int NX, int LINES, int MODE>
+template <int NX, int LINES, int MODE, int XS>
 __device__ __forceinline__ void real_space32(cf* u, cf* d, const PassXArgs& a, const float* fbuf, int line, int t,
                                              const LaneCoef& lc, double& su, double& sd) {
   // tier of the warp (bounds as in pass_x.cuh, row_tier): n_up + n_dn <= NT at every point of the thread
@@ -103,20 +105,22 @@ __device__ __forceinline__ void real_space32(cf* u, cf* d, const PassXArgs& a, c
   if (__all_sync(0xffffffffu, ph_ok && z <= SPGPE_Z_MICRO)) tier = 0;
   // two series tiers are enough here (degree 2 and degree 7): the fp32 path is not bound by this arithmetic
   if (bz0) {
-    if (tier == 0) real_space32_tier<NX, LINES, MODE, 0, true>(u, d, a, fbuf, line, t, lc, su, sd);
-    else if (tier == 2) real_space32_tier<NX, LINES, MODE, 2, true>(u, d, a, fbuf, line, t, lc, su, sd);
-    else real_space32_tier<NX, LINES, MODE, 3, true>(u, d, a, fbuf, line, t, lc, su, sd);
+    if (tier == 0) real_space32_tier<NX, LINES, MODE, 0, true, XS>(u, d, a, fbuf, line, t, lc, su, sd);
+    else if (tier == 2) real_space32_tier<NX, LINES, MODE, 2, true, XS>(u, d, a, fbuf, line, t, lc, su, sd);
+    else real_space32_tier<NX, LINES, MODE, 3, true, XS>(u, d, a, fbuf, line, t, lc, su, sd);
   } else {
-    if (tier == 0) real_space32_tier<NX, LINES, MODE, 0, false>(u, d, a, fbuf, line, t, lc, su, sd);
-    else if (tier == 2) real_space32_tier<NX, LINES, MODE, 2, false>(u, d, a, fbuf, line, t, lc, su, sd);
-    else real_space32_tier<NX, LINES, MODE, 3, false>(u, d, a, fbuf, line, t, lc, su, sd);
+    if (tier == 0) real_space32_tier<NX, LINES, MODE, 0, false, XS>(u, d, a, fbuf, line, t, lc, su, sd);
+    else if (tier == 2) real_space32_tier<NX, LINES, MODE, 2, false, XS>(u, d, a, fbuf, line, t, lc, su, sd);
+    else real_space32_tier<NX, LINES, MODE, 3, false, XS>(u, d, a, fbuf, line, t, lc, su, sd);
   }
 }
 
 // ---- row pass ---------------------------------------------------------------------------------------------------
-// MODE_PRO / MODE_MID / MODE_EPI as in pass_x.cuh; rows only (xs = 1).  a.tw32: two-float twiddles of NX.
-template <int NX, int LINES, int MODE>
-__global__ void __launch_bounds__(LINES * (NX / 16), Lines32<NX>::XCTAS) row32_kernel(const PassXArgs a) {
+// MODE_PRO / MODE_MID / MODE_EPI as in pass_x.cuh.  XS = 1: a line is a row.  XS = 2 (LINES = 2): the two lines are the
+// even and the odd points of one row of 2 NX points (split x axis).  a.tw32: two-float twiddles of NX.
+template <int NX, int LINES, int MODE, int XS>
+__global__ void __launch_bounds__(LINES * (NX / 16), (LINES * (NX / 16) <= 256) ? 2 : 1) row32_kernel(const PassXArgs a) {
+  static_assert(XS == 1 || LINES == 2, "a split row is handled as its two interleaved lines");
   typedef Plan<NX> P;
   typedef Smem32<NX, LINES> SM;
   extern __shared__ __align__(128) float4 smem4[];
@@ -166,11 +170,10 @@ __global__ void __launch_bounds__(LINES * (NX / 16), Lines32<NX>::XCTAS) row32_k
     if (tid == 0) next_s[it & 1] = nxt;
     mbar_wait(&full, it & 1);
     {
-      const float4* row = stg + (size_t)line * NX;
 #pragma unroll
       for (int n = 0; n < 16; ++n) {
         const int x = (MODE == MODE_PRO) ? (t + n * T) : stored_pos32<NX>(t, n);
-        lds4(row, x, u[n], d[n]);
+        lds4(stg, XS == 1 ? line * NX + x : 2 * x + line, u[n], d[n]);
       }
     }
     if (MODE == MODE_PRO && a.scale != nullptr) {
@@ -208,7 +211,7 @@ __global__ void __launch_bounds__(LINES * (NX / 16), Lines32<NX>::XCTAS) row32_k
     else fields_hook();
     mbar_wait(&ffull, it & 1);
     if (a.V == nullptr || a.Om == nullptr || a.De == nullptr) __syncthreads();  // zero fills are per-thread writes
-    real_space32<NX, LINES, MODE>(u, d, a, fbuf, line, t, lc, su, sd);
+    real_space32<NX, LINES, MODE, XS>(u, d, a, fbuf, line, t, lc, su, sd);
     if (MODE == MODE_EPI && a.want_norm) {
 #pragma unroll
       for (int m = 16; m >= 1; m >>= 1) {
@@ -235,15 +238,19 @@ __global__ void __launch_bounds__(LINES * (NX / 16), Lines32<NX>::XCTAS) row32_k
       issue_loads(nxt_grp);
       nxt = sched_next(a.sched);
     }
-    float4* dst = reinterpret_cast<float4*>(a.dst) + ((size_t)grp * LINES + line) * NX;
+    float4* dst = reinterpret_cast<float4*>(a.dst) + (size_t)grp * LINES * NX;  // first point of the group's rows
     if (MODE == MODE_EPI) {
 #pragma unroll
-      for (int n = 0; n < 16; ++n) dst[t + n * T] = make_float4(u[n].re, u[n].im, d[n].re, d[n].im);
+      for (int n = 0; n < 16; ++n)
+        dst[XS == 1 ? line * NX + (t + n * T) : 2 * (t + n * T) + line] = make_float4(u[n].re, u[n].im, d[n].re, d[n].im);
     } else {
       dft_lastf<-1, P::RL>(u);
       dft_lastf<-1, P::RL>(d);
 #pragma unroll
-      for (int n = 0; n < 16; ++n) dst[stored_pos32<NX>(t, n)] = make_float4(u[n].re, u[n].im, d[n].re, d[n].im);
+      for (int n = 0; n < 16; ++n) {
+        const int x = stored_pos32<NX>(t, n);
+        dst[XS == 1 ? line * NX + x : 2 * x + line] = make_float4(u[n].re, u[n].im, d[n].re, d[n].im);
+      }
     }
     grp = nxt_grp;
   }
@@ -289,7 +296,9 @@ __global__ void __launch_bounds__(LINES * (NX / 16), Lines32<NX>::XCTAS) row32_k
 // YMODE_STEP: psi^(k_x, y) -> F_y -> * ex_c(k_x) ey(k_y) -> F_y^-1 -> psi^(k_x, y), in place, LINES adjacent columns per
 // CTA, thread index = line + LINES * t.  a.tw32: two-float twiddles of NY; a.eyk32 [NY], a.exk32 [2][nx]: two-float
 // phase tables (hi.re, hi.im, lo.re, lo.im); a.tmap32: box [min(NY, 256) rows][LINES points].
-template <int NY, int LINES>
+// YMODE_FWDONLY / YMODE_INVONLY (split transforms, api.cu): forward transform only, results in stored order / inverse
+// transform only, input in stored order.  YMODE_STEP with a.exk32 == NULL applies the k_y factor alone (split x axis).
+template <int NY, int LINES, int YMODE>
 __global__ void __launch_bounds__(LINES * (NY / 16), (LINES * (NY / 16) <= 256) ? 2 : 1) col32_kernel(const __grid_constant__ PassYArgs a) {
   typedef Plan<NY> P;
   typedef Smem32<NY, LINES> SM;
@@ -332,6 +341,7 @@ __global__ void __launch_bounds__(LINES * (NY / 16), (LINES * (NY / 16) <= 256) 
   __syncthreads();
   cf u[16], d[16];
   int it = 0;
+  TL_DECL(8);
   for (int grp = blockIdx.x; grp < ngroups; ++it) {
     const size_t col = (size_t)grp * LINES + line;
     if (tid == 0) {
@@ -342,19 +352,30 @@ __global__ void __launch_bounds__(LINES * (NY / 16), (LINES * (NY / 16) <= 256) 
       }
     }
     mbar_wait(&mbar, it & 1);
+    TL_MARK(0);
 #pragma unroll
-    for (int n = 0; n < 16; ++n) lds4(stg, (t + n * T) * LINES + line, u[n], d[n]);
+    for (int n = 0; n < 16; ++n)
+      lds4(stg, (YMODE == YMODE_INVONLY ? stored_pos32<NY>(t, n) : t + n * T) * LINES + line, u[n], d[n]);
     __syncthreads();  // every thread has taken its staged values: the buffers may be overwritten
-    line_fwd32<NY, LINEW, LASTW>(buf, twS, t, u, d);
-    {
-      const float4 xu = __ldg(a.exk32 + col), xd = __ldg(a.exk32 + (size_t)a.nx + col);
+    TL_MARK(1);
+    if (YMODE != YMODE_INVONLY) line_fwd32<NY, LINEW, LASTW>(buf, twS, t, u, d);
+    TL_MARK(2);
+    if (YMODE == YMODE_STEP) {
+      const bool has_x = a.exk32 != nullptr;
+      const float4 one = make_float4(1.f, 0.f, 0.f, 0.f);
+      const float4 xu = has_x ? __ldg(a.exk32 + col) : one, xd = has_x ? __ldg(a.exk32 + (size_t)a.nx + col) : one;
 #pragma unroll
       for (int r = 0; r < 16; ++r) {
         const float4 f = __ldg(a.eyk32 + stored_pos32<NY>(t, r));
-        u[r] = cmul2(cmul2(u[r], f.x, f.y, f.z, f.w), xu.x, xu.y, xu.z, xu.w);
-        d[r] = cmul2(cmul2(d[r], f.x, f.y, f.z, f.w), xd.x, xd.y, xd.z, xd.w);
+        u[r] = cmul2(u[r], f.x, f.y, f.z, f.w);
+        d[r] = cmul2(d[r], f.x, f.y, f.z, f.w);
+        if (has_x) {
+          u[r] = cmul2(u[r], xu.x, xu.y, xu.z, xu.w);
+          d[r] = cmul2(d[r], xd.x, xd.y, xd.z, xd.w);
+        }
       }
     }
+    TL_MARK(3);
     int nxt_grp = ngroups;
     auto hook = [&]() {
       __syncthreads();  // last read of the line buffers done by every warp: the next tile may land
@@ -364,12 +385,23 @@ __global__ void __launch_bounds__(LINES * (NY / 16), (LINES * (NY / 16) <= 256) 
         nxt = sched_next(a.sched);
       }
     };
-    line_inv32<NY, LINEW, LASTW>(buf, twS, t, u, d, hook);
-    float4* dst = reinterpret_cast<float4*>(a.psi) + (size_t)t * a.nx + col;
+    float4* dst = reinterpret_cast<float4*>(a.psi) + col;
+    if (YMODE == YMODE_FWDONLY) {
+      hook();
 #pragma unroll
-    for (int n = 0; n < 16; ++n) dst[(size_t)n * T * a.nx] = make_float4(u[n].re, u[n].im, d[n].re, d[n].im);
+      for (int n = 0; n < 16; ++n)
+        dst[(size_t)stored_pos32<NY>(t, n) * a.nx] = make_float4(u[n].re, u[n].im, d[n].re, d[n].im);
+    } else {
+      line_inv32<NY, LINEW, LASTW>(buf, twS, t, u, d, hook);
+      TL_MARK(4);
+#pragma unroll
+      for (int n = 0; n < 16; ++n) dst[(size_t)(t + n * T) * a.nx] = make_float4(u[n].re, u[n].im, d[n].re, d[n].im);
+    }
+    TL_MARK(5);
+    TL_TILE();
     grp = nxt_grp;
   }
+  TL_DUMP("col32 wait|stage|fwd|phase|inv|store", 6);
   if (tid == 0) sched_finish(a.sched);
 }
 
