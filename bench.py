@@ -328,12 +328,16 @@ def run_ours(args, wname):
         step_bytes = (bytes_pt[0] + bytes_pt[1]) * P
         flops_pt = 20.0 * np.log2(float(P)) + 360.0
         dfma_tf = sp.spgpe_probe_dfma(stream.cuda_stream)
+        ffma_tf = sp.spgpe_probe_ffma(stream.cuda_stream)
         traffic, traffic_src = read_traffic(w.name, ["pass_x_kernel", "pass_y_kernel"][dom])
         line = {
             "metric": METRIC, "value": world * P * K / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
             "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic",
+            "dtype": "f64" if spec["dtype"] == "c128" else "f32", "data": "synthetic",
             "config": {"workload": w.name, "grid": [w.nx, w.ny], "storage": spec["dtype"],
+                       "arithmetic": "fp64 throughout" if spec["dtype"] == "c128" else
+                                     "fp32 transforms with two-float twiddles and phase factors, fp64 per-point "
+                                     "2x2 exponential and reductions (DESIGN.md R-14)",
                        "time": "imaginary" if imag else "real", "dt": dt, "parallelism": "replicas only",
                        "l2": f"state {psi_bytes >> 20} MiB + fields {(nfields * P * rsz) >> 20} MiB per replica; "
                              + ("larger than the 126 MB L2, no flush" if psi_bytes > 126e6 else
@@ -343,7 +347,8 @@ def run_ours(args, wname):
             "steps_per_s": world * K / (ms * 1e-3),
             "step_hbm_gbs": step_bytes / (ms / K * 1e-3) / 1e9,
             "step_roofline_frac": step_bytes / (ms / K * 1e-3) / 1e9 / peak,
-            "roofline": {"bound": "hbm", "kernel": ["pass_x_kernel (row pass)", "pass_y_kernel (column pass)"][dom],
+            "roofline": {"bound": "hbm", "kernel": ["row pass (pass_x_kernel / row32_kernel)",
+                                                    "column pass (pass_y_db_kernel / col32_kernel)"][dom],
                          "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": traffic, "traffic_source": traffic_src,
                          "algorithmic_bytes": bytes_pt[dom] * P, "peak_source": peak_src,
@@ -355,6 +360,12 @@ def run_ours(args, wname):
                               "unit": "TFLOP/s", "frac": flops_pt * P / (ms / K * 1e-3) / 1e12 / dfma_tf,
                               "flops_per_point_step": flops_pt,
                               "peak_source": "measured in this run (DFMA loop, 2 flops per FMA)"},
+            **({} if spec["dtype"] == "c128" else {
+                # complex64: the transforms' flops (20 log2 P per point and step) against the measured fp32 FMA peak
+                "roofline_fp32": {"bound": "alu", "achieved": 20.0 * np.log2(float(P)) * P / (ms / K * 1e-3) / 1e12,
+                                  "peak": ffma_tf, "unit": "TFLOP/s",
+                                  "frac": 20.0 * np.log2(float(P)) * P / (ms / K * 1e-3) / 1e12 / ffma_tf,
+                                  "peak_source": "measured in this run (FFMA loop, 2 flops per FMA)"}}),
             "e2e": {"value": world * P * K / e2e_s, "unit": UNIT,
                     "h2d_bytes_per_step": (psi_bytes + nfields * P * rsz) / K, "d2h_bytes_per_step": psi_bytes / K,
                     "job": f"fields + psi host->device, spgpe_step({K}), psi device->host; {e2e_s:.4f} s"},

@@ -41,7 +41,7 @@ extern "C" {
 
 typedef struct spgpe_ctx* spgpe_handle; /* opaque */
 
-enum { SPGPE_C128 = 0, SPGPE_C64 = 1 }; /* storage precision of psi and fields (arithmetic is fp64) */
+enum { SPGPE_C128 = 0, SPGPE_C64 = 1 }; /* storage precision of psi and fields; arithmetic: DESIGN.md R-14 */
 enum { SPGPE_NORM_PER_COMPONENT = 0, SPGPE_NORM_TOTAL = 1 }; /* R-7 */
 enum { SPGPE_RS_EXPONENTIAL = 0, SPGPE_RS_NESTED = 1 };      /* form of the real-space part R(tau), R-5 / R-15 */
 
@@ -147,9 +147,10 @@ const char* spgpe_strerror(int code);
 const char* spgpe_last_cuda_error(void);
 
 /* Measurement helpers (not part of the method): peak probes used for bench.py's roofline denominators.
- * spgpe_probe_dfma: sustained fp64 FMA rate of the device in TFLOP/s (2 flops per FMA).
+ * spgpe_probe_dfma / spgpe_probe_ffma: sustained fp64 / fp32 FMA rate of the device in TFLOP/s (2 flops per FMA).
  * spgpe_probe_copy: device-to-device copy bandwidth in GB/s (read + write bytes) over `bytes` bytes. */
 int spgpe_probe_dfma(void* cuda_stream, double* tflops);
+int spgpe_probe_ffma(void* cuda_stream, double* tflops);
 int spgpe_probe_copy(void* cuda_stream, long long bytes, double* gbs);
 
 #ifdef __cplusplus

@@ -32,7 +32,7 @@ ABI_SYMBOLS = (
     "spgpe_step", "spgpe_step_observe", "spgpe_set_real_space_split", "spgpe_set_annealing",
     "spgpe_norm", "spgpe_energy", "spgpe_synchronize", "spgpe_launch_count",
     "spgpe_profile", "spgpe_profile_read",
-    "spgpe_strerror", "spgpe_last_cuda_error", "spgpe_probe_dfma", "spgpe_probe_copy",
+    "spgpe_strerror", "spgpe_last_cuda_error", "spgpe_probe_dfma", "spgpe_probe_ffma", "spgpe_probe_copy",
 )
 
 
@@ -86,6 +86,7 @@ def lib() -> ctypes.CDLL:
         L.spgpe_strerror.restype = ctypes.c_char_p
         L.spgpe_last_cuda_error.restype = ctypes.c_char_p
         L.spgpe_probe_dfma.argtypes = [vp, ctypes.POINTER(cd)]
+        L.spgpe_probe_ffma.argtypes = [vp, ctypes.POINTER(cd)]
         L.spgpe_probe_copy.argtypes = [vp, ctypes.c_longlong, ctypes.POINTER(cd)]
         _lib = L
     return _lib
@@ -264,6 +265,12 @@ def spgpe_profile_read(h: Handle):
 def spgpe_probe_dfma(stream: Optional[int] = None) -> float:
     out = ctypes.c_double()
     _check(lib().spgpe_probe_dfma(ctypes.c_void_p(stream or 0), ctypes.byref(out)))
+    return out.value
+
+
+def spgpe_probe_ffma(stream: Optional[int] = None) -> float:
+    out = ctypes.c_double()
+    _check(lib().spgpe_probe_ffma(ctypes.c_void_p(stream or 0), ctypes.byref(out)))
     return out.value
 
 

@@ -704,6 +704,11 @@ extern "C" int spgpe_probe_dfma(void* cuda_stream, double* tflops) {
   CK(aux_probe_dfma((cudaStream_t)cuda_stream, tflops));
   return SPGPE_OK;
 }
+extern "C" int spgpe_probe_ffma(void* cuda_stream, double* tflops) {
+  if (!tflops) return SPGPE_ERR_INVALID_ARG;
+  CK(aux_probe_ffma((cudaStream_t)cuda_stream, tflops));
+  return SPGPE_OK;
+}
 extern "C" int spgpe_probe_copy(void* cuda_stream, long long bytes, double* gbs) {
   if (!gbs || bytes <= 0) return SPGPE_ERR_INVALID_ARG;
   CK(aux_probe_copy((cudaStream_t)cuda_stream, bytes, gbs));

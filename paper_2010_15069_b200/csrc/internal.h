@@ -85,6 +85,7 @@ cudaError_t aux_set_targets(double* target, double n_up, double n_dn, cudaStream
 cudaError_t aux_absmax(int dt, const void* field, size_t points, double* out, cudaStream_t s);
 // probes (bench roofline denominators)
 cudaError_t aux_probe_dfma(cudaStream_t s, double* tflops);
+cudaError_t aux_probe_ffma(cudaStream_t s, double* tflops);
 cudaError_t aux_probe_copy(cudaStream_t s, long long bytes, double* gbs);
 
 }  // namespace spgpe
