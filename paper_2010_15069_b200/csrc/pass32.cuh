@@ -167,7 +167,17 @@ __global__ void __launch_bounds__(LINES * (NX / 16), (LINES * (NX / 16) <= 256) 
   cf u[16], d[16];
   int it = 0;
   for (int grp = blockIdx.x; grp < ngroups; ++it) {
-    if (tid == 0) next_s[it & 1] = nxt;
+    if (tid == 0) {
+      next_s[it & 1] = nxt;
+      // one CTA per SM (512 threads): nothing else covers the next group's load, so it is asked into L2 a whole
+      // period ahead (with two CTAs per SM the other CTA covers it and the prefetch only costs, as in pass_x.cuh)
+      if (NTHR > 256 && nxt < ngroups) {
+        prefetch_l2_bulk(reinterpret_cast<const char*>(a.src) + (size_t)nxt * GROUP_BYTES, GROUP_BYTES);
+        if (a.V) prefetch_l2_bulk(reinterpret_cast<const char*>(a.V) + (size_t)nxt * FIELD_BYTES, FIELD_BYTES);
+        if (a.Om) prefetch_l2_bulk(reinterpret_cast<const char*>(a.Om) + (size_t)nxt * FIELD_BYTES, FIELD_BYTES);
+        if (a.De) prefetch_l2_bulk(reinterpret_cast<const char*>(a.De) + (size_t)nxt * FIELD_BYTES, FIELD_BYTES);
+      }
+    }
     mbar_wait(&full, it & 1);
     {
 #pragma unroll

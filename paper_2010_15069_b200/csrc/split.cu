@@ -26,10 +26,17 @@ __global__ void __launch_bounds__(256) split_kernel(const SplitArgs a) {
 #pragma unroll
     for (int j = 0; j < SY; ++j)
 #pragma unroll
-      for (int i = 0; i < SX; ++i)
+      for (int i = 0; i < SX; ++i) {
+        const size_t pt = ((size_t)py * SY + j) * a.nx + (size_t)px * SX + i;
+        if (DT == 1) {  // complex64 storage: both components of a point in one 16-byte access
+          const float4 q = __ldcs(reinterpret_cast<const float4*>(a.psi) + pt);
+          u[j][i][0] = mk((double)q.x, (double)q.y);
+          u[j][i][1] = mk((double)q.z, (double)q.w);
+        } else {
 #pragma unroll
-        for (int c = 0; c < 2; ++c)
-          u[j][i][c] = St::ld(a.psi, (((size_t)py * SY + j) * a.nx + (size_t)px * SX + i) * 2 + c);
+          for (int c = 0; c < 2; ++c) u[j][i][c] = St::ld(a.psi, pt * 2 + c);
+        }
+      }
     // true frequencies of the block: f + ax m along a split axis; along an unsplit axis the stored position itself
     // indexes the (stored-order) tables
     const int fx = SX == 2 ? a.fx[px] : px, fy = SY == 2 ? a.fy[py] : py;
@@ -113,10 +120,16 @@ __global__ void __launch_bounds__(256) split_kernel(const SplitArgs a) {
 #pragma unroll
     for (int j = 0; j < SY; ++j)
 #pragma unroll
-      for (int i = 0; i < SX; ++i)
+      for (int i = 0; i < SX; ++i) {
+        const size_t pt = ((size_t)py * SY + j) * a.nx + (size_t)px * SX + i;
+        if (DT == 1) {
+          reinterpret_cast<float4*>(a.psi)[pt] = make_float4((float)u[j][i][0].re, (float)u[j][i][0].im,
+                                                             (float)u[j][i][1].re, (float)u[j][i][1].im);
+        } else {
 #pragma unroll
-        for (int c = 0; c < 2; ++c)
-          St::st(a.psi, (((size_t)py * SY + j) * a.nx + (size_t)px * SX + i) * 2 + c, u[j][i][c]);
+          for (int c = 0; c < 2; ++c) St::st(a.psi, pt * 2 + c, u[j][i][c]);
+        }
+      }
   }
   if (ENERGY) {
     __shared__ double red[8];
