@@ -66,10 +66,10 @@ cudaError_t launch_pdl(K kernel, int grid, int threads, size_t smem, cudaStream_
 }
 
 // grid_out: number of CTAs launched (= rows of PassXArgs::partial written by MODE_EPI)
-template <int DT, int N, int MODE, int XS, bool NEST>
-cudaError_t launch_x_xs(const PassXArgs& a, int ny, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
+template <int DT, int N, int MODE, int XS, bool NEST, int TIME>
+cudaError_t launch_x_time(const PassXArgs& a, int ny, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
   constexpr int L = Lines<N>::X;
-  auto k = pass_x_kernel<DT, N, L, MODE, XS, NEST>;
+  auto k = pass_x_kernel<DT, N, L, MODE, XS, NEST, TIME>;
   constexpr size_t smem = XSmem<N, L>::BYTES;
   static int cache[SPGPE_MAX_DEVICES] = {};
   int resident = 0;
@@ -79,6 +79,16 @@ cudaError_t launch_x_xs(const PassXArgs& a, int ny, cudaStream_t s, const Launch
   const int grid = groups < resident ? groups : resident;
   *grid_out = grid;
   return launch_pdl(k, grid, L * (N / 8), smem, s, a);
+}
+
+// real or imaginary time is a compile-time property of the default opening / closing passes (TIME = 0 | 1); the
+// steady-state pass exists in real time only; the nested instantiations decide at run time (TIME = 2)
+template <int DT, int N, int MODE, int XS, bool NEST>
+cudaError_t launch_x_xs(const PassXArgs& a, int ny, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
+  if constexpr (NEST) return launch_x_time<DT, N, MODE, XS, true, 2>(a, ny, s, env, grid_out);
+  else if constexpr (MODE == MODE_MID || MODE == MODE_FWD) return launch_x_time<DT, N, MODE, XS, false, 0>(a, ny, s, env, grid_out);
+  else return a.imag ? launch_x_time<DT, N, MODE, XS, false, 1>(a, ny, s, env, grid_out)
+                     : launch_x_time<DT, N, MODE, XS, false, 0>(a, ny, s, env, grid_out);
 }
 
 template <int DT, int N, int MODE>

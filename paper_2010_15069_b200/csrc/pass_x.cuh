@@ -153,7 +153,8 @@ __device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, siz
 // component at its own point), evaluates the half-step(s) in the (mine, other) basis (su2.cuh, LaneCoef) and
 // sends the other component back.  Fields come from shared memory (stage_fields), index lx = line*NX + x.
 // TIER: evaluation tier of su2.cuh, guaranteed by the caller for every point of the warp.
-template <int DT, int NX, int LINES, int MODE, int TIER, bool BZ0>
+// TIME: 0 real time, 1 imaginary time (both known at compile time: the default kernels), 2 decided by a.imag at run time
+template <int DT, int NX, int LINES, int MODE, int TIER, bool BZ0, int TIME>
 __device__ __forceinline__ void real_space_tier(cplx* v, const PassXArgs& a, const void* fbuf, int line, int t, int c,
                                                 const LaneCoef& lc, double& sm, double& so, ObsSums& ob) {
   typedef Store<DT> St;
@@ -187,7 +188,7 @@ __device__ __forceinline__ void real_space_tier(cplx* v, const PassXArgs& a, con
       double pr, pi;
       phase_eval<TIER>((a1 + a2) * tau, pr, pi);
       apply_phase(m, o[i], pr, pi);
-    } else if (a.imag) {
+    } else if (TIME == 2 ? (a.imag != 0) : (TIME == 1)) {
       const double a1 = su2_apply<true, TIER, BZ0>(m, o[i], Vv, hO, hD, tau, tau2, lc);
       const double e = exp(-a1 * tau);
       m = mk(m.re * e, m.im * e);
@@ -295,7 +296,7 @@ __device__ __forceinline__ bool nested_fast(const cplx* v, const PassXArgs& a, c
   return __all_sync(0xffffffffu, ok);
 }
 
-template <int DT, int NX, int LINES, int MODE, bool NEST>
+template <int DT, int NX, int LINES, int MODE, bool NEST, int TIME>
 __device__ __forceinline__ void real_space(cplx* v, const PassXArgs& a, const void* fbuf, int line, int t, int c,
                                            const LaneCoef& lc, double& sm, double& so, ObsSums& ob) {
   if constexpr (NEST) {
@@ -308,15 +309,15 @@ __device__ __forceinline__ void real_space(cplx* v, const PassXArgs& a, const vo
   const bool bz0 = a.hc.cb_u == 0.0 && a.hc.cb_d == 0.0;
   const int tier = row_tier<MODE>(v, a, lc, bz0 && MODE == MODE_MID);
   if (bz0) {  // all g equal: b_z has no density term
-    if (tier == 0) real_space_tier<DT, NX, LINES, MODE, 0, true>(v, a, fbuf, line, t, c, lc, sm, so, ob);
-    else if (tier == 1) real_space_tier<DT, NX, LINES, MODE, 1, true>(v, a, fbuf, line, t, c, lc, sm, so, ob);
-    else if (tier == 2) real_space_tier<DT, NX, LINES, MODE, 2, true>(v, a, fbuf, line, t, c, lc, sm, so, ob);
-    else real_space_tier<DT, NX, LINES, MODE, 3, true>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    if (tier == 0) real_space_tier<DT, NX, LINES, MODE, 0, true, TIME>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    else if (tier == 1) real_space_tier<DT, NX, LINES, MODE, 1, true, TIME>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    else if (tier == 2) real_space_tier<DT, NX, LINES, MODE, 2, true, TIME>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    else real_space_tier<DT, NX, LINES, MODE, 3, true, TIME>(v, a, fbuf, line, t, c, lc, sm, so, ob);
   } else {
-    if (tier == 0) real_space_tier<DT, NX, LINES, MODE, 0, false>(v, a, fbuf, line, t, c, lc, sm, so, ob);
-    else if (tier == 1) real_space_tier<DT, NX, LINES, MODE, 1, false>(v, a, fbuf, line, t, c, lc, sm, so, ob);
-    else if (tier == 2) real_space_tier<DT, NX, LINES, MODE, 2, false>(v, a, fbuf, line, t, c, lc, sm, so, ob);
-    else real_space_tier<DT, NX, LINES, MODE, 3, false>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    if (tier == 0) real_space_tier<DT, NX, LINES, MODE, 0, false, TIME>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    else if (tier == 1) real_space_tier<DT, NX, LINES, MODE, 1, false, TIME>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    else if (tier == 2) real_space_tier<DT, NX, LINES, MODE, 2, false, TIME>(v, a, fbuf, line, t, c, lc, sm, so, ob);
+    else real_space_tier<DT, NX, LINES, MODE, 3, false, TIME>(v, a, fbuf, line, t, c, lc, sm, so, ob);
   }
 }
 
@@ -331,7 +332,8 @@ struct XSmem {
 // one (psi rows and field rows) is requested into L2, so that its loads find the data there.
 // NEST: the real-space part is the nested split (PassXArgs::nest; its own instantiation, so that the default kernels
 // keep their register budget)
-template <int DT, int NX, int LINES, int MODE, int XS, bool NEST>
+// TIME: see real_space_tier (the nested instantiations keep the run-time switch)
+template <int DT, int NX, int LINES, int MODE, int XS, bool NEST, int TIME>
 __global__ void __launch_bounds__(LINES * (NX / 8), (LINES * (NX / 8) <= 256) ? 2 : 1)
 pass_x_kernel(const PassXArgs a) {
   typedef Plan<NX> P;
@@ -381,9 +383,11 @@ pass_x_kernel(const PassXArgs a) {
     } else {
       const size_t lb = line_base(grp * LINES + line);
       if (MODE == MODE_PRO || MODE == MODE_FWD) {
+        // slot n holds point t + n T of BOTH lanes of a pair (one contiguous 32-byte point per pair and copy); the odd
+        // lane, which keeps its points rotated by 8, takes register n out of slot (n + 8) mod 16 (staged())
 #pragma unroll
         for (int n = 0; n < 16; ++n)
-          cp_async_elem(stg + n * NTHR + tid, src + (lb + (size_t)(t + ((n + 8 * c) & 15) * T) * S) * 2 + c);
+          cp_async_elem(stg + n * NTHR + tid, src + (lb + (size_t)(t + n * T) * S) * 2 + c);
       } else {
 #pragma unroll
         for (int g = 0; g < P::G; ++g)
@@ -402,6 +406,7 @@ pass_x_kernel(const PassXArgs a) {
       const int g = n / P::RL, s = n % P::RL;
       return St::cv(row[((t + g * T) + (NX / P::RL) * s) * 2 + c]);
     } else {
+      if (MODE == MODE_PRO || MODE == MODE_FWD) return St::cv(stg[((n + 8 * c) & 15) * NTHR + tid]);
       return St::cv(stg[n * NTHR + tid]);
     }
   };
@@ -447,12 +452,12 @@ pass_x_kernel(const PassXArgs a) {
     if (BULK) mbar_wait(&full, it & 1);
 #pragma unroll
     for (int n = 0; n < 16; ++n) v[n] = staged(n);
-    if (MODE == MODE_PRO && a.scale != nullptr) {
+    if (MODE == MODE_PRO && TIME != 0 && a.scale != nullptr) {
       const double s = a.scale[c];
 #pragma unroll
       for (int n = 0; n < 16; ++n) v[n] = mk(v[n].re * s, v[n].im * s);
     }
-    if (MODE == MODE_PRO && a.anneal_event > 0) {
+    if (MODE == MODE_PRO && TIME != 0 && a.anneal_event > 0) {
 #pragma unroll 1
       for (int n = 0; n < 16; ++n) {
         // register n holds point t + ((n + 8c) mod 16) T of the line (same index as the load above)
@@ -484,7 +489,7 @@ pass_x_kernel(const PassXArgs a) {
       // complete on the mbarrier every thread has just waited on
       if (!FBULK || a.V == nullptr || a.Om == nullptr || a.De == nullptr) __syncthreads();
       TL_MARK(2);
-      real_space<DT, NX, LINES, MODE, NEST>(v, a, smem, line, t, c, lc, sm, so, ob);
+      real_space<DT, NX, LINES, MODE, NEST, TIME>(v, a, smem, line, t, c, lc, sm, so, ob);
       TL_MARK(3);
       if (mode_is_epi(MODE) && (a.want_norm || MODE == MODE_EPI_OBS)) {
         // norm partials of this row group, one slot per group: the sums do not depend on which CTA took the group,
@@ -533,8 +538,13 @@ pass_x_kernel(const PassXArgs a) {
       if (tid == 0) nxt = sched_next(a.sched);  // consumed in the next iteration
     }
     if (mode_is_epi(MODE)) {
+      // point m = t + m T is written by both lanes of a pair at once (one full 32-byte point): the odd lane holds it in
+      // register (m + 8) mod 16
 #pragma unroll
-      for (int n = 0; n < 16; ++n) St::st(a.dst, (lbase + (size_t)(t + ((n + 8 * c) & 15) * T) * S) * 2 + c, v[n]);
+      for (int m = 0; m < 16; ++m) {
+        const cplx val = c ? v[(m + 8) & 15] : v[m];
+        St::st(a.dst, (lbase + (size_t)(t + m * T) * S) * 2 + c, val);
+      }
     } else {
       dft_last<-1, P::RL>(v);
       TL_MARK(5);
@@ -552,6 +562,8 @@ pass_x_kernel(const PassXArgs a) {
     grp = nxt_grp;
   }
   if (MODE == MODE_MID) TL_DUMP("xmid wait+stage|inv|fields|real|fwd|issue+last|ex+store", 7);
+  if (MODE == MODE_PRO) TL_DUMP("xpro wait+stage|inv|fields|real|fwd|issue+last|ex+store", 7);
+  if (MODE == MODE_EPI) TL_DUMP("xepi wait+stage|inv|fields|real|fwd|issue+last|ex+store", 7);
   if (mode_is_epi(MODE)) {
     // imaginary time (a6): the CTA that finishes last turns the per-group norm partials into the rescale factors
     // of the next step (fixed summation order), so no separate kernel is needed
