@@ -19,7 +19,7 @@ namespace spgpe {
 
 // rows per CTA of the fp32 row pass / columns per CTA of the fp32 column pass (threads = lines * N / 16)
 template <int N> struct Lines32 {
-  static constexpr int X = (N >= 2048) ? 2 : (N == 1024 ? 4 : (N == 512 ? 8 : 16));
+  static constexpr int X = (N == 4096) ? 2 : (N == 2048) ? 1 : (N == 1024 ? 4 : (N == 512 ? 8 : 16));
   static constexpr int Y = (N >= 1024) ? 2 : (N == 512 ? 4 : (N == 256 ? 2 : 4));
   static constexpr int XCTAS = (N == 4096) ? 1 : 2;  // resident CTAs per SM the row pass is compiled for
 };
@@ -119,7 +119,7 @@ __device__ __forceinline__ void real_space32(cf* u, cf* d, const PassXArgs& a, c
 // MODE_PRO / MODE_MID / MODE_EPI as in pass_x.cuh.  XS = 1: a line is a row.  XS = 2 (LINES = 2): the two lines are the
 // even and the odd points of one row of 2 NX points (split x axis).  a.tw32: two-float twiddles of NX.
 template <int NX, int LINES, int MODE, int XS>
-__global__ void __launch_bounds__(LINES * (NX / 16), (LINES * (NX / 16) <= 256) ? 2 : 1) row32_kernel(const PassXArgs a) {
+__global__ void __launch_bounds__(LINES * (NX / 16), (LINES * (NX / 16) <= 128) ? 3 : (LINES * (NX / 16) <= 256) ? 2 : 1) row32_kernel(const PassXArgs a) {
   static_assert(XS == 1 || LINES == 2, "a split row is handled as its two interleaved lines");
   typedef Plan<NX> P;
   typedef Smem32<NX, LINES> SM;
