@@ -46,7 +46,7 @@ struct spgpe_ctx {
   int tab_imag;
   bool tab_valid;
   double *partial, *scale, *target, *dout;
-  CUtensorMap tmap_psi, tmap_scratch, tmap_psi_db, tmap_psi_duo, tmap_psi32;  // column-pass tensor maps of psi / the energy scratch buffer
+  CUtensorMap tmap_psi, tmap_scratch, tmap_psi_db, tmap_psi32;  // column-pass tensor maps of psi / the energy scratch buffer
   int* sched;    // [4] work counters of the persistent kernels: row pass [0..1], column pass [2..3]
   double2 *wcx, *wcy;         // split axes: join twiddles
   int *fpx, *fpy;             // split axes: true frequency of a sub-transform position
@@ -369,7 +369,6 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
   if (e == cudaSuccess) e = make_col_tmap(h, h->psi, plan_lines_y(h->my), &h->tmap_psi);
   if (e == cudaSuccess && h->f32_ok) e = make_col_tmap(h, h->psi, plan_lines_y32(h->my), &h->tmap_psi32);
   if (e == cudaSuccess && plan_lines_ydb(h->my) > 0) e = make_col_tmap(h, h->psi, plan_lines_ydb(h->my), &h->tmap_psi_db);
-  if (e == cudaSuccess && plan_has_duo(h->my) && h->dt == SPGPE_C128) e = make_col_tmap(h, h->psi, 1, &h->tmap_psi_duo, h->my / 16);
   if (e != cudaSuccess) {
     spgpe_destroy(h);
     return e == cudaErrorMemoryAllocation ? SPGPE_ERR_NO_MEMORY : cuda_fail(e);
@@ -532,7 +531,7 @@ static int step_impl(spgpe_handle h, int n, double dt, int imag, bool obs) {
   ya.tw32 = h->tw_y32; ya.eyk32 = h->eyk32; ya.tmap32 = h->tmap_psi32;
   ya.exk32 = (h->sx == 1 && h->sy == 1) ? h->exk32 : nullptr;
   // the k_x phase rides on the column pass unless a split axis sends the k-space phases to the join kernel
-  ya.exk = (h->sx == 1 && h->sy == 1) ? h->exk : nullptr; ya.sched = h->sched + 2; ya.tmap = h->tmap_psi; ya.tmap_db = h->tmap_psi_db; ya.tmap_duo = h->tmap_psi_duo;
+  ya.exk = (h->sx == 1 && h->sy == 1) ? h->exk : nullptr; ya.sched = h->sched + 2; ya.tmap = h->tmap_psi; ya.tmap_db = h->tmap_psi_db;
   // the observed column pass (last step only): k-space sums per CTA into kpartial
   auto last_kspace = [&]() -> cudaError_t {
     if (!obs) return kspace_part(h, ya);

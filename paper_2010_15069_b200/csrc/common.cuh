@@ -33,7 +33,7 @@ namespace spgpe {
 struct LaunchEnv {
   int device;        // CUDA device ordinal of the handle
   int ctas_per_sm;   // SPGPE_DEBUG_CTAS_PER_SM: cap on resident CTAs per SM of the persistent kernels (0: none)
-  int no_ydb;        // SPGPE_DEBUG_NO_YDB: column pass without the double-buffered kernel
+  int no_ydb;        // SPGPE_DEBUG_NO_YDB=1: column pass on the two-column kernel instead of the double-buffered one
   int xdbg;          // SPGPE_DEBUG_X: experiment switches of the row pass
 };
 

@@ -55,7 +55,6 @@ cudaError_t launch_split(int dt, const SplitArgs& a, int sx, int sy, int energy,
 int plan_tw_total(int n);                       // number of twiddle entries of length n
 void plan_fill_twiddles(int n, double2* host);  // exp(-2 pi i k lo / (16 M_j)) blocks, see common.cuh
 int plan_lines_ydb(int n);                      // columns per tile of the double-buffered column pass (0: none)
-bool plan_has_duo(int n);                       // a two-group column pass exists for length n (complex128)
 int plan_lines_x(int n);                        // rows per CTA of the row pass of length n
 int plan_lines_y(int n);                        // columns per CTA of the column pass of length n
 int plan_lines_x32(int n);                      // rows / columns per CTA of the fp32 kernels (pass32.cuh)

@@ -12,7 +12,6 @@ template <int N> struct Lines {
   static constexpr int X = (N >= 2048) ? 1 : (N == 1024 ? 2 : 4);
   static constexpr int Y = (N >= 4096) ? 1 : (N >= 1024 ? 2 : 4);
   static constexpr int YDB = (N == 2048) ? 1 : (N == 1024 ? 2 : 0);  // columns per tile of pass_y_db_kernel (0: none)
-  static constexpr bool DUO = (N == 2048);  // pass_y_duo_kernel (two independent 256-thread groups per CTA)
 };
 
 constexpr int SPGPE_MAX_DEVICES = 64;
@@ -131,47 +130,11 @@ cudaError_t launch_y_db(const PassYArgs& a, cudaStream_t s, const LaunchEnv& env
   *grid_out = grid;
   return launch_pdl(k, grid, L * (N / 8), smem, s, a);
 }
-// experiment: one column per 256-thread CTA, two CTAs per SM (k_y phases from global memory), tensor map of the
-// double-buffered kernel (same box)
-template <int DT, int N>
-cudaError_t launch_y_2cta(PassYArgs a, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
-  auto k = pass_y_kernel<DT, N, 1, YMODE_STEP, true>;
-  constexpr size_t smem = YSmem<N, 1, true>::BYTES;
-  static int cache[SPGPE_MAX_DEVICES] = {};
-  int resident = 0;
-  cudaError_t e = resident_ctas(k, N / 8, smem, env, cache, &resident);
-  if (e != cudaSuccess) return e;
-  a.tmap = a.tmap_db;
-  const int groups = a.nx;
-  const int grid = groups < resident ? groups : resident;
-  *grid_out = grid;
-  return launch_pdl(k, grid, N / 8, smem, s, a);
-}
-template <int N, bool STG>
-cudaError_t launch_y_duo(const PassYArgs& a, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
-  auto k = pass_y_duo_kernel<N, STG>;
-  constexpr size_t smem = YSmemDuo<N>::BYTES;
-  static int cache[SPGPE_MAX_DEVICES] = {};
-  int resident = 0;
-  cudaError_t e = resident_ctas(k, N / 4, smem, env, cache, &resident);
-  if (e != cudaSuccess) return e;
-  const int pairs = (a.nx + 1) / 2;
-  const int grid = pairs < resident ? pairs : resident;
-  *grid_out = grid;
-  return launch_pdl(k, grid, N / 4, smem, s, a);
-}
 // YMODE_STEP goes to the double-buffered kernel where one exists.  complex64 storage keeps the two-column kernel:
 // a one-column tile of float2 pairs is only 16 bytes wide, too narrow for efficient TMA boxes (measured at 2048^2:
 // 86 us against 78 us).
 template <int DT, int N>
 cudaError_t launch_y_step(const PassYArgs& a, cudaStream_t s, const LaunchEnv& env, int* g) {
-  if constexpr (N == 2048 && DT == 0) {
-    if (env.no_ydb == 2) return launch_y_2cta<DT, N>(a, s, env, g);
-  }
-  if constexpr (Lines<N>::DUO && DT == 0) {
-    if (env.no_ydb == 3) return launch_y_duo<N, false>(a, s, env, g);
-    if (env.no_ydb == 4) return launch_y_duo<N, true>(a, s, env, g);
-  }
   if constexpr (Lines<N>::YDB > 0 && DT == 0) {
     if (!env.no_ydb) return launch_y_db<DT, N>(a, s, env, g);
   }

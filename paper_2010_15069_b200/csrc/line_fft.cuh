@@ -122,60 +122,6 @@ __device__ __forceinline__ void lds_stage(const double2* buf, int t, int c, cplx
   }
 }
 
-// ---- "dense in block" layout (three-stage plans) ---------------------------------------------------------------
-// The padded index above is block-local: with B = N/16 points per block (the sub-transforms after stage 1) and
-// BS = B + (B >> PADSHIFT), point p = b*B + r lives at (b*BS + r + (r >> PADSHIFT))*2 + c.  The dense-in-block
-// variant drops the inner padding, (b*BS + r)*2 + c: every block keeps its footprint, and a block of B consecutive
-// points is contiguous, which is how a TMA box lands (or leaves).  The exchange between stage 1 and stage 2 is
-// conflict-free in this layout too, and stage 1 reads and writes the SAME addresses (positions n*B + t, n = 0..15),
-// so a tile that lands dense-in-block needs no staging copy and no barrier in front of the first exchange:
-// pass_y_duo_kernel (pass_y.cuh) uses it for landing, first/last exchange and output.
-template <int N>
-struct DenseBlock {
-  static constexpr int B = N / 16;
-  static constexpr int BS = B + (B >> Plan<N>::PADSHIFT);
-};
-// stage 1: register n <-> point n*B + t
-template <int N>
-__device__ __forceinline__ void lds_dense1(const double2* buf, int t, int c, cplx* v) {
-  const double2* p = buf + t * 2 + c;
-#pragma unroll
-  for (int n = 0; n < 16; ++n) {
-    const double2 d = p[n * (DenseBlock<N>::BS * 2)];
-    v[n] = mk(d.x, d.y);
-  }
-}
-template <int N>
-__device__ __forceinline__ void sts_dense1(double2* buf, int t, int c, const cplx* v) {
-  double2* p = buf + t * 2 + c;
-#pragma unroll
-  for (int n = 0; n < 16; ++n) p[n * (DenseBlock<N>::BS * 2)] = make_double2(v[n].re, v[n].im);
-}
-// stage 2: thread t = hi*M2 + lo, register n <-> point hi*B + n*M2 + lo (block hi)
-template <int N>
-__device__ __forceinline__ int dense2_base(int t, int c) {
-  constexpr int M2 = N >> 8;
-  const int lo = t & (M2 - 1), hi = t / M2;
-  return (hi * DenseBlock<N>::BS + lo) * 2 + c;
-}
-template <int N>
-__device__ __forceinline__ void lds_dense2(const double2* buf, int t, int c, cplx* v) {
-  constexpr int M2 = N >> 8;
-  const double2* p = buf + dense2_base<N>(t, c);
-#pragma unroll
-  for (int n = 0; n < 16; ++n) {
-    const double2 d = p[n * (M2 * 2)];
-    v[n] = mk(d.x, d.y);
-  }
-}
-template <int N>
-__device__ __forceinline__ void sts_dense2(double2* buf, int t, int c, const cplx* v) {
-  constexpr int M2 = N >> 8;
-  double2* p = buf + dense2_base<N>(t, c);
-#pragma unroll
-  for (int n = 0; n < 16; ++n) p[n * (M2 * 2)] = make_double2(v[n].re, v[n].im);
-}
-
 // v[k] *= w_j[k][lo] (forward) or conj (inverse); w_j[k][lo] = exp(-2 pi i k lo / (16 M_j))
 //
 // flip (0 or 0x80000000, stage 1 only) negates the twiddles of odd k.  With it a thread may hold its 16 points

@@ -39,7 +39,6 @@ struct PassYArgs {
   // psi as a 2-D tensor [NY rows][4 nx reals], box = [min(NY, 256) rows][4 LINES reals]: the columns of a group
   CUtensorMap tmap;
   CUtensorMap tmap_db;  // the same tensor with the box of the double-buffered kernel (pass_y_db_kernel)
-  CUtensorMap tmap_duo; // the same tensor, box = [NY/16 rows][one column] (pass_y_duo_kernel)
   CUtensorMap tmap32;   // the same tensor with the tile of col32_kernel (pass32.cuh)
 };
 
@@ -424,174 +423,6 @@ __global__ void __launch_bounds__(LINES * (NY / 8), 1) pass_y_db_kernel(const __
     tma_store_wait_all();
     sched_finish(a.sched);
   }
-}
-
-// ---- two-group variant of YMODE_STEP (complex128, three-stage plans) ------------------------------------------
-// One 512-thread CTA per SM; its two halves ("groups" of 256 threads) work on different columns, independently of
-// each other: every group has its own line buffer, its own named barrier (bar.sync id, 256), its own mbarrier and
-// takes its tiles from the common work counter.  While one group exchanges through shared memory the other one
-// runs butterflies, so the FP64 pipe and the shared-memory pipe of the SM are busy at the same time (a single
-// group alternates between them).  The two groups share the twiddle and k_y tables, which is what lets two line
-// buffers fit one SM.
-// A group's line buffer is also where its tile lands and leaves (TMA, dense in block: line_fft.cuh): stage 1
-// reads the landed values and writes the exchange into the same addresses, the inverse transform's last stage
-// writes the results where the TMA store picks them up, so a tile costs three group barriers and no staging copy.
-// The load of the next tile is issued by the group's first thread once the store has read the buffer; the tile
-// was requested into L2 a period earlier (TMA prefetch), so that this exposed load is short, and the other group
-// has the SM to itself meanwhile.
-template <int NY>
-struct YSmemDuo {
-  static constexpr int EBUF = Plan<NY>::PTS * 2;  // one line buffer, double2 elements
-  static constexpr int TW = tw_total<NY>();
-  static constexpr size_t BYTES = (size_t)(2 * EBUF + TW + NY) * 16;
-  static constexpr bool FITS = BYTES <= 227u * 1024u;
-};
-
-__device__ __forceinline__ void bar_sync_named(int id, int nthreads) {
-  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
-
-// STG: results leave with plain 16-byte stores from registers (no TMA store, the line buffer is free one stage earlier)
-template <int NY, bool STG>
-__global__ void __launch_bounds__(NY / 4, 1) pass_y_duo_kernel(const __grid_constant__ PassYArgs a) {
-  typedef Plan<NY> P;
-  typedef YSmemDuo<NY> SM;
-  typedef DenseBlock<NY> DB;
-  static_assert(P::NS == 3, "built for three-stage plans");
-  extern __shared__ __align__(128) double2 smem[];
-  constexpr int T = P::T;
-  constexpr int GT = NY / 8;   // threads per group
-  constexpr int NTHR = 2 * GT;
-  constexpr unsigned TILE_BYTES = (unsigned)NY * 32u;
-  const int tid = threadIdx.x;
-  const int grp_id = tid / GT;  // 0 or 1
-  const int gt = tid % GT;
-  const int c = gt & 1;
-  const int t = gt >> 1;
-  double2* buf = smem + (size_t)grp_id * SM::EBUF;
-  double2* twS = smem + 2 * SM::EBUF;
-  double2* eyS = twS + SM::TW;
-  __shared__ __align__(8) unsigned long long mbar[2];
-  __shared__ int next_s[2][2];
-  unsigned long long* full = &mbar[grp_id];
-  pdl_launch_dependents();
-  copy_table_async(twS, a.tw, SM::TW, tid, NTHR);
-  copy_table_async(eyS, a.eyk, NY, tid, NTHR);  // written before any pass kernel started (see pass_y_kernel)
-  const int ncols = a.nx;
-  auto issue_loads = [&](int col) {  // the group's first thread only: 16 boxes of one block each, dense in block
-    fence_proxy_async();
-    mbar_expect_tx(full, TILE_BYTES);
-#pragma unroll
-    for (int b = 0; b < 16; ++b) tma_load_2d(buf + (size_t)b * DB::BS * 2, &a.tmap_duo, col * 4, b * DB::B, full);
-  };
-  auto prefetch_l2 = [&](int col) {
-#pragma unroll
-    for (int b = 0; b < 16; ++b) tma_prefetch_2d(&a.tmap_duo, col * 4, b * DB::B);
-  };
-  if (tid == 0) {
-    mbar_init(&mbar[0], 1);
-    mbar_init(&mbar[1], 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  pdl_wait();
-  cp_async_wait_all();
-  __syncthreads();  // tables and barriers are visible to every thread
-  // Work distribution: the 2 * gridDim.x groups are the workers; worker w starts with column w and then takes
-  // 2 * gridDim.x + (counter value).  `nxt` (group's first thread) is the column after the current one, fetched one
-  // tile ahead so that the atomic's latency never sits in front of a barrier.
-  const int worker = 2 * (int)blockIdx.x + grp_id;
-  const int nworkers = 2 * (int)gridDim.x;
-  auto take = [&]() { return nworkers + atomicAdd(&a.sched[0], 1); };
-  int nxt = ncols;
-  if (gt == 0 && worker < ncols) {
-    issue_loads(worker);
-    nxt = take();
-    if (nxt < ncols) prefetch_l2(nxt);
-  }
-  cplx v[16];
-  int it = 0;
-  TL_DECL(8);
-  for (int col = worker; col < ncols; ++it) {
-    const double2 exv = a.exk != nullptr ? __ldg(a.exk + (size_t)c * ncols + col) : make_double2(1.0, 0.0);
-    if (gt == 0) next_s[grp_id][it & 1] = nxt;  // read by the group behind the forward transform's barrier
-    mbar_wait(full, it & 1);
-    TL_MARK(0);
-    // ---- forward transform: stage 1 in place on the landed tile
-    lds_dense1<NY>(buf, t, c, v);
-    dft16<-1>(v);
-    twiddle<NY, 1, -1>(twS, t, v, 0);
-    sts_dense1<NY>(buf, t, c, v);
-    bar_sync_named(1 + grp_id, GT);
-    lds_dense2<NY>(buf, t, c, v);
-    dft16<-1>(v);
-    twiddle<NY, 2, -1>(twS, t, v, 0);
-    __syncwarp();  // the block's dense reads are done before its padded writes alias them
-    sts_stage<NY, 2>(buf, t, c, v);
-    __syncwarp();
-    lds_last<NY>(buf, t, c, v);
-    dft_last<-1, P::RL>(v);
-    TL_MARK(1);
-    // ---- k-space factor ex_c(k_x) ey(k_y)
-#pragma unroll
-    for (int g = 0; g < P::G; ++g)
-#pragma unroll
-      for (int s = 0; s < P::RL; ++s) {
-        const double2 f = eyS[(t + g * T) + (NY / P::RL) * s];
-        v[g * P::RL + s] = cmul(cmul(v[g * P::RL + s], mk(f.x, f.y)), mk(exv.x, exv.y));
-      }
-    TL_MARK(2);
-    // ---- inverse transform, mirror image
-    dft_last<+1, P::RL>(v);
-    sts_last<NY>(buf, t, c, v);
-    __syncwarp();
-    lds_stage<NY, 2>(buf, t, c, v);
-    twiddle<NY, 2, +1>(twS, t, v, 0);
-    dft16<+1>(v);
-    __syncwarp();  // the block's padded reads are done before its dense writes alias them
-    sts_dense2<NY>(buf, t, c, v);
-    bar_sync_named(1 + grp_id, GT);
-    const int nxt_col = next_s[grp_id][it & 1];
-    lds_dense1<NY>(buf, t, c, v);
-    if (STG) {
-      bar_sync_named(1 + grp_id, GT);  // every thread of the group has done its last read of the line buffer
-      TL_MARK(3);
-      if (gt == 0 && nxt_col < ncols) {
-        issue_loads(nxt_col);
-        nxt = take();
-        if (nxt < ncols) prefetch_l2(nxt);
-      }
-      twiddle<NY, 1, +1>(twS, t, v, 0);
-      dft16<+1>(v);
-      double2* g = reinterpret_cast<double2*>(a.psi) + ((size_t)t * ncols + col) * 2 + c;
-#pragma unroll
-      for (int n = 0; n < 16; ++n) g[(size_t)n * T * ncols * 2] = make_double2(v[n].re, v[n].im);
-    } else {
-      twiddle<NY, 1, +1>(twS, t, v, 0);
-      dft16<+1>(v);
-      sts_dense1<NY>(buf, t, c, v);  // results, dense in block: what the TMA store reads
-      fence_proxy_async();
-      bar_sync_named(1 + grp_id, GT);
-      TL_MARK(3);
-      if (gt == 0) {
-#pragma unroll
-        for (int b = 0; b < 16; ++b) tma_store_2d(&a.tmap_duo, col * 4, b * DB::B, buf + (size_t)b * DB::BS * 2);
-        tma_store_commit();
-        if (nxt_col < ncols) {
-          tma_store_wait_read();  // the buffer has been read: the next tile may land
-          issue_loads(nxt_col);
-          nxt = take();
-          if (nxt < ncols) prefetch_l2(nxt);
-        }
-      }
-    }
-    TL_MARK(4);
-    TL_TILE();
-    col = nxt_col;
-  }
-  TL_DUMP("yduo wait|fwd|ey|inv|store+issue", 5);
-  if (gt == 0) tma_store_wait_all();
-  __syncthreads();
-  if (tid == 0) sched_finish(a.sched);
 }
 
 }  // namespace spgpe

@@ -61,7 +61,6 @@ int plan_lines_y32(int n) {
 }
 int plan_lines_ydb(int n) { return n == 2048 ? Lines<2048>::YDB : (n == 1024 ? Lines<1024>::YDB : 0); }
 
-bool plan_has_duo(int n) { return n == 2048 ? Lines<2048>::DUO : (n == 1024 ? Lines<1024>::DUO : false); }
 
 int plan_tw_total(int n) {
   PlanInfo p = plan_info(n);
