@@ -229,3 +229,22 @@ def test_fp32_and_fp64_arithmetic_kernels_agree_and_mix(sp, monkeypatch):
         assert_parity(out[mode], ref, TOL_C64)
     assert np.abs(out["0"] - out["1"]).max() / np.abs(ref).max() < 2e-5
     assert np.abs(out["0"] - out["1"]).max() > 0  # they are different kernels
+
+
+@pytest.mark.parametrize("split_min,nx,ny", [(128, 128, 256), (128, 1024, 64), (1024, 1024, 1024), (1024, 2048, 256),
+                                             (1024, 64, 1024)])
+@pytest.mark.parametrize("imag", [0, 1])
+def test_fp32_path_with_split_axes(sp, monkeypatch, split_min, nx, ny, imag):
+    """Split axes of complex64 grids (SPGPE_DEBUG_SPLIT_MIN forces them at small sizes): sub-lines of 512 points and
+    more run on the fp32 row kernel as the even / odd points of a row, shorter ones on the fp64-arithmetic kernel; the
+    column pass runs forward-only / inverse-only around the join kernel; the energy call keeps its own path."""
+    monkeypatch.setenv("SPGPE_DEBUG_SPLIT_MIN", str(split_min))
+    psi, V, Om, De, p, _ = random_problem(nx, ny, seed=nx + ny)
+    psi32 = np.ascontiguousarray(psi, dtype=np.complex64).astype(np.complex128)
+    V, Om, De = _f32(V), _f32(Om), _f32(De)
+    h = make_solver(sp, psi32, V, Om, De, p, dtype="c64")
+    sp.spgpe_step(h, 4, 1e-3, imag)
+    ref = orc.step(psi32, V, Om, De, p, 4, 1e-3, imag)
+    assert_parity(sp.spgpe_get_psi_host(h), ref, TOL_C64)
+    e_ref = orc.energy(ref, V, Om, De, p)
+    assert np.abs(sp.spgpe_energy(h) - e_ref).max() < 1e-5 * np.abs(e_ref).max()
