@@ -52,7 +52,8 @@ enum {
   SPGPE_ERR_NOT_READY = -3,   /* step/norm/energy/get before set_psi */
   SPGPE_ERR_CUDA = -4,        /* a CUDA call failed; spgpe_last_cuda_error() gives its text */
   SPGPE_ERR_NO_DEVICE = -5,   /* no CUDA device / not an sm_100 device */
-  SPGPE_ERR_NO_MEMORY = -6    /* host or device allocation failed in spgpe_create */
+  SPGPE_ERR_NO_MEMORY = -6,   /* host or device allocation failed in spgpe_create */
+  SPGPE_ERR_TOO_LARGE = -7    /* spgpe_norm_noalloc: nx or ny beyond its fixed maximum of 8192 */
 };
 
 typedef struct {
@@ -129,6 +130,20 @@ int spgpe_step_observe(spgpe_handle h, int n, double dt, int imag, double h_out[
 
 /* N_c = dx dy sum_r |psi_c|^2 (R-8); out = {N_up, N_dn}; synchronises. */
 int spgpe_norm(spgpe_handle h, double out[2]);
+/* The same norms N_c = dx dy sum_r |psi_c|^2 (R-8) WITHOUT a handle and without any allocation, for callers that
+ * cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).
+ *   d_psi : DEVICE pointer, complex [ny][nx][2] of `dtype` (SPGPE_C128 | SPGPE_C64), caller-owned, read only;
+ *   d_out : DEVICE pointer to 2 doubles {N_up, N_dn}, caller-owned, written asynchronously on `cuda_stream`
+ *           (a cudaStream_t, NULL = the default stream) of the CURRENT device; the call does not synchronise.
+ * Limit: 1 <= nx, ny <= 8192 (no power-of-two requirement); anything larger returns SPGPE_ERR_TOO_LARGE and touches
+ * nothing.  The reduction's scratch (1024 x 2 partial sums, 16 KiB) is a fixed device array inside the library that
+ * every GPU loading the library holds until the process exits; its address is looked up once per device on the first
+ * call there (make that call outside a graph capture).  All calls on a device share that array: calls that overlap on
+ * the GPU (two streams, two host threads) race on it -- keep them on one stream or order them with events.  No slot of
+ * it has to be cleared between calls (each call overwrites every slot before reading it).  Calls no cudaMalloc,
+ * cudaFree or allocating library routine.  Same summation order as spgpe_norm (bit-identical results). */
+int spgpe_norm_noalloc(const void* d_psi, int dtype, int nx, int ny, double Lx, double Ly, double* d_out,
+                       void* cuda_stream);
 /* Energy functional implied by Eqs. 4-8 (R-8), totals not per particle:
  * out = {total, kinetic, potential+Zeeman, interaction, Raman}; synchronises. */
 int spgpe_energy(spgpe_handle h, double out[5]);

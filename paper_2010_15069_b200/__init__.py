@@ -30,7 +30,7 @@ ABI_SYMBOLS = (
     "spgpe_set_potential_host", "spgpe_set_raman_host", "spgpe_set_zeeman_host",
     "spgpe_set_psi", "spgpe_get_psi", "spgpe_set_psi_host", "spgpe_get_psi_host", "spgpe_set_norm_targets",
     "spgpe_step", "spgpe_step_observe", "spgpe_set_real_space_split", "spgpe_set_annealing",
-    "spgpe_norm", "spgpe_energy", "spgpe_synchronize", "spgpe_launch_count",
+    "spgpe_norm", "spgpe_norm_noalloc", "spgpe_energy", "spgpe_synchronize", "spgpe_launch_count",
     "spgpe_profile", "spgpe_profile_read",
     "spgpe_strerror", "spgpe_last_cuda_error", "spgpe_probe_dfma", "spgpe_probe_ffma", "spgpe_probe_copy",
 )
@@ -77,6 +77,7 @@ def lib() -> ctypes.CDLL:
         L.spgpe_set_real_space_split.argtypes = [vp, ci]
         L.spgpe_set_annealing.argtypes = [vp, ci, cd, ctypes.c_ulonglong]
         L.spgpe_norm.argtypes = [vp, ctypes.POINTER(cd)]
+        L.spgpe_norm_noalloc.argtypes = [vp, ci, ci, ci, cd, cd, vp, vp]
         L.spgpe_energy.argtypes = [vp, ctypes.POINTER(cd)]
         L.spgpe_launch_count.argtypes = [vp]
         L.spgpe_launch_count.restype = ctypes.c_longlong
@@ -233,6 +234,26 @@ def spgpe_norm(h: Handle) -> np.ndarray:
     out = (ctypes.c_double * 2)()
     _check(lib().spgpe_norm(h.ptr, out))
     return np.array(out[:])
+
+
+def spgpe_norm_noalloc(psi, Lx: float, Ly: float, out, stream: Optional[int] = None) -> None:
+    """N_up, N_dn of the torch CUDA tensor psi (complex [ny, nx, 2]) into the torch CUDA tensor out (2 float64), on
+    `stream` (cudaStream_t as an integer; None = default), without a handle and without any allocation; asynchronous.
+    Sizes beyond 8192 per axis raise SpgpeError (code -7).  Argument marshalling only (include/spgpe.h)."""
+    import torch
+    if not (hasattr(psi, "is_cuda") and psi.is_cuda and psi.dim() == 3 and psi.shape[2] == 2 and psi.is_contiguous()):
+        raise TypeError("psi: contiguous torch CUDA tensor of shape [ny, nx, 2]")
+    if psi.dtype == torch.complex128:
+        dt = SPGPE_C128
+    elif psi.dtype == torch.complex64:
+        dt = SPGPE_C64
+    else:
+        raise TypeError("psi: complex128 or complex64")
+    if not (hasattr(out, "is_cuda") and out.is_cuda and out.dtype == torch.float64 and out.numel() == 2
+            and out.is_contiguous() and out.device == psi.device):
+        raise TypeError("out: contiguous torch CUDA tensor of 2 float64 on psi's device")
+    _check(lib().spgpe_norm_noalloc(psi.data_ptr(), dt, int(psi.shape[1]), int(psi.shape[0]), float(Lx), float(Ly),
+                                    out.data_ptr(), ctypes.c_void_p(stream or 0)))
 
 
 def spgpe_energy(h: Handle) -> np.ndarray:

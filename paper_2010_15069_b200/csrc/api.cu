@@ -693,6 +693,7 @@ extern "C" const char* spgpe_strerror(int code) {
     case SPGPE_ERR_CUDA: return "CUDA error (see spgpe_last_cuda_error)";
     case SPGPE_ERR_NO_DEVICE: return "no sm_100 CUDA device";
     case SPGPE_ERR_NO_MEMORY: return "out of host or device memory";
+    case SPGPE_ERR_TOO_LARGE: return "size beyond the fixed maximum of the no-allocation entry point (nx, ny <= 8192)";
     default: return "unknown error code";
   }
 }
