@@ -85,42 +85,65 @@ static __device__ __noinline__ cplx anneal_noise(const PassXArgs& a, unsigned lo
   return mk(r * cn, r * sn);
 }
 
-// Copy the three field rows of this CTA's LINES rows into shared memory ([field][line][x], working precision); a NULL
-// field is filled with zeros.  Every thread of the CTA takes part.  Rows (XS == 1) are contiguous: thread 0 issues one
-// bulk copy per field (completion on `bar`, evict-first in L2: the fields are read once per pass and must not push
+// Field rows in shared memory: [field][line][x] in working precision, with a gap of 64 bytes in the middle of every
+// row.  The two lanes of a pair read different halves of the row (x = t + i T and x = t + (i + 8) T, T = NX/16): without
+// the gap the halves are a multiple of 128 bytes apart and the two lanes of every pair hit the same banks (measured:
+// every field read took twice its wavefronts, 1.2 M conflict wavefronts per launch at 2048^2, all of the row pass's
+// bank conflicts); with it the second half sits 16 banks further and a warp's read is conflict-free.
+template <int DT, int NX, int LINES>
+struct FieldLayout {
+  typedef typename Store<DT>::real real;
+  static constexpr int GAP = 64 / (int)sizeof(real);                 // elements
+  static constexpr int ROW = NX + GAP;                               // elements of a staged row
+  static constexpr int FIELD = LINES * ROW;                          // elements of a staged field
+  static constexpr int HALF_BYTES = (NX / 2) * (int)sizeof(real);    // bytes of half a row
+  static constexpr int ROW_BYTES = NX * (int)sizeof(real);
+  static __device__ __forceinline__ int at(int line, int x) { return line * ROW + x + (x >= NX / 2 ? GAP : 0); }
+};
+
+// Copy the three field rows of this CTA's LINES rows into shared memory (FieldLayout); a NULL field is filled with
+// zeros.  Every thread of the CTA takes part.  Rows (XS == 1) are contiguous: thread 0 issues two bulk copies per field
+// and row (the two halves; completion on `bar`, evict-first in L2: the fields are read once per pass and must not push
 // the order parameter out); the strided lines of a split axis take one cp.async per real.
 template <int DT, int NX, int LINES, int XS>
 __device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, size_t first_point, int first_line,
                                              int tid, unsigned long long* bar, bool fbulk) {
   typedef typename Store<DT>::real real;
-  constexpr int FIELD_BYTES = LINES * NX * (int)sizeof(real);
+  typedef FieldLayout<DT, NX, LINES> FL;
+  constexpr int FIELD_BYTES = LINES * NX * (int)sizeof(real);   // bytes copied per field
   constexpr int NCH = FIELD_BYTES / 16;
+  constexpr int PAD_BYTES = FL::FIELD * (int)sizeof(real);      // bytes a staged field occupies
   constexpr int NTHR = LINES * (NX / 8);
   const void* src[3] = {a.V, a.Om, a.De};
+  auto zero_fill = [&](int f) {
+    char* dst = reinterpret_cast<char*>(fbuf) + f * PAD_BYTES;
+    for (int k = tid; k < PAD_BYTES / 16; k += NTHR) *reinterpret_cast<float4*>(dst + k * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
+  };
   if constexpr (XS != 1) {  // strided lines: one cp.async per real
     constexpr int S = XS;
 #pragma unroll
     for (int f = 0; f < 3; ++f) {
-      real* dst = reinterpret_cast<real*>(fbuf) + f * (LINES * NX);
+      real* dst = reinterpret_cast<real*>(fbuf) + f * FL::FIELD;
       const real* g = reinterpret_cast<const real*>(src[f]);
+      if (g == nullptr) { zero_fill(f); continue; }
       for (int k = tid; k < LINES * NX; k += NTHR) {
-        const int L = first_line + k / NX, pos = k % NX;
-        if (g != nullptr) cp_async_real(dst + k, g + (size_t)(L / S) * NX * S + (size_t)pos * S + (L % S));
-        else dst[k] = (real)0;
+        const int l = k / NX, L = first_line + l, pos = k % NX;
+        cp_async_real(dst + FL::at(l, pos), g + (size_t)(L / S) * NX * S + (size_t)pos * S + (L % S));
       }
     }
   } else if (!fbulk) {
 #pragma unroll
     for (int f = 0; f < 3; ++f) {
-      char* dst = reinterpret_cast<char*>(fbuf) + f * FIELD_BYTES;
+      char* dst = reinterpret_cast<char*>(fbuf) + f * PAD_BYTES;
       if (src[f] != nullptr) {
         const char* g = reinterpret_cast<const char*>(src[f]) + first_point * sizeof(real);
 #pragma unroll
-        for (int k = tid; k < NCH; k += NTHR) cp_async16(dst + k * 16, g + k * 16);
+        for (int k = tid; k < NCH; k += NTHR) {
+          const int l = (k * 16) / FL::ROW_BYTES, off = (k * 16) % FL::ROW_BYTES;
+          cp_async16(dst + l * (FL::ROW * (int)sizeof(real)) + off + (off >= FL::HALF_BYTES ? 64 : 0), g + k * 16);
+        }
       } else {
-#pragma unroll
-        for (int k = tid; k < NCH; k += NTHR)
-          *reinterpret_cast<float4*>(dst + k * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
+        zero_fill(f);
       }
     }
   } else {
@@ -131,19 +154,20 @@ __device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, siz
       mbar_expect_tx(bar, n * (unsigned)FIELD_BYTES);  // n == 0: the phase completes at once
 #pragma unroll
       for (int f = 0; f < 3; ++f)
-        if (src[f] != nullptr)
-          bulk_load_1d_hint(reinterpret_cast<char*>(fbuf) + f * FIELD_BYTES,
-                            reinterpret_cast<const char*>(src[f]) + first_point * sizeof(real), FIELD_BYTES, bar, policy);
+        if (src[f] != nullptr) {
+          const char* g = reinterpret_cast<const char*>(src[f]) + first_point * sizeof(real);
+          char* dst = reinterpret_cast<char*>(fbuf) + f * PAD_BYTES;
+#pragma unroll
+          for (int l = 0; l < LINES; ++l)
+#pragma unroll
+            for (int hf = 0; hf < 2; ++hf)
+              bulk_load_1d_hint(dst + l * (FL::ROW * (int)sizeof(real)) + hf * (FL::HALF_BYTES + 64),
+                                g + l * FL::ROW_BYTES + hf * FL::HALF_BYTES, FL::HALF_BYTES, bar, policy);
+        }
     }
 #pragma unroll
-    for (int f = 0; f < 3; ++f) {
-      if (src[f] == nullptr) {
-        char* dst = reinterpret_cast<char*>(fbuf) + f * FIELD_BYTES;
-#pragma unroll
-        for (int k = tid; k < NCH; k += NTHR)
-          *reinterpret_cast<float4*>(dst + k * 16) = make_float4(0.f, 0.f, 0.f, 0.f);
-      }
-    }
+    for (int f = 0; f < 3; ++f)
+      if (src[f] == nullptr) zero_fill(f);
   }
 }
 
@@ -151,7 +175,7 @@ __device__ __forceinline__ void stage_fields(void* fbuf, const PassXArgs& a, siz
 // thread position t holds in v[i], i < 8, its component at "its" points x = t + (i + 8c) T and in v[8 + i] its
 // component at the partner lane's points.  For point i a lane receives the partner's v[8 + i] (the other
 // component at its own point), evaluates the half-step(s) in the (mine, other) basis (su2.cuh, LaneCoef) and
-// sends the other component back.  Fields come from shared memory (stage_fields), index lx = line*NX + x.
+// sends the other component back.  Fields come from shared memory (stage_fields, FieldLayout).
 // TIER: evaluation tier of su2.cuh, guaranteed by the caller for every point of the warp.
 // TIME: 0 real time, 1 imaginary time (both known at compile time: the default kernels), 2 decided by a.imag at run time
 template <int DT, int NX, int LINES, int MODE, int TIER, bool BZ0, int TIME>
@@ -160,9 +184,10 @@ __device__ __forceinline__ void real_space_tier(cplx* v, const PassXArgs& a, con
   typedef Store<DT> St;
   typedef typename St::real real;
   constexpr int T = NX / 16;
-  const real* fV = reinterpret_cast<const real*>(fbuf) + line * NX + t + 8 * c * T;
-  const real* fO = fV + LINES * NX;
-  const real* fD = fO + LINES * NX;
+  typedef FieldLayout<DT, NX, LINES> FL;
+  const real* fV = reinterpret_cast<const real*>(fbuf) + line * FL::ROW + t + c * (8 * T + FL::GAP);
+  const real* fO = fV + FL::FIELD;
+  const real* fD = fO + FL::FIELD;
   const double tau = a.tau, tau2 = a.tau * a.tau;
   // the other component of the lane's 8 points arrives first (one batch of shuffles), then the points are
   // evaluated without touching the shuffle / shared-memory path, then the other component goes back in one batch
@@ -243,9 +268,10 @@ __device__ __forceinline__ void real_space_nested(cplx* v, const PassXArgs& a, c
   typedef Store<DT> St;
   typedef typename St::real real;
   constexpr int T = NX / 16;
-  const real* fV = reinterpret_cast<const real*>(fbuf) + line * NX + t + 8 * c * T;
-  const real* fO = fV + LINES * NX;
-  const real* fD = fO + LINES * NX;
+  typedef FieldLayout<DT, NX, LINES> FL;
+  const real* fV = reinterpret_cast<const real*>(fbuf) + line * FL::ROW + t + c * (8 * T + FL::GAP);
+  const real* fO = fV + FL::FIELD;
+  const real* fD = fO + FL::FIELD;
   const double tau = a.tau, th = 0.5 * a.tau;
   cplx o[8];
 #pragma unroll
