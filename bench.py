@@ -14,6 +14,9 @@ A "step" is one Strang step of the whole hot path (a6
   roofline   : dominant kernel (the longer of the row pass and the column pass), timed per launch with CUDA
                events on the handle's stream (spgpe_profile) over a second region of K steps.
   cpu_baseline: the oracle as it stands, on this box's host cores, a bounded sample of the same workload.
+  cufft_comparison: context only -- the paper's own formulation (torch.fft.fft2 = cuFFT, Hadamard products as torch
+               elementwise operations) timed on this GPU for the same workload, and the relative L2 difference between
+               the library and that independent GPU path after the same steps (N = 1, states up to 256 MiB).
 Multi-GPU: replicas only: every rank steps its own copy of the workload, no collective
 on the data path; value = N * P * K / max-over-ranks time.
 --impl reference times the oracle (oracle/) on the host cores; rank 0 only.
@@ -167,6 +170,81 @@ def oracle_sample(w_cfg: int, dtype: str, budget_s: float, steps: int, threads: 
             f"config {w_cfg}'s recipe on a {n}x{n} grid (full size {full}x{full}), "
             f"{'imaginary' if imag else 'real'} time")
     return n * n / sec, threads, what, sec
+
+
+def cufft_comparison(w, spec, steps: int, warmup: int, ours_after_steps=None):
+    """The paper's own formulation of the same step, timed on this GPU as CONTEXT (BASELINE.json north_star: "a
+    cuFFT-plus-elementwise-kernel version of the same step may be timed as a comparison"; PyTorch
+    arrays, torch.fft (cuFFT) and Hadamard products): torch.fft.fft2 / ifft2 on a [2, ny, nx] array, the k-space phase
+    and the closed 2x2 real-space factor as plain torch elementwise operations.  Not part of the product path and not
+    the oracle; bench.py only.  Returns a dict for the JSON line.  ours_after_steps: the library's psi (numpy
+    [ny, nx, 2]) after `steps` steps from the same initial state, for a cross-check of the two GPU paths."""
+    import torch
+    dev = torch.device("cuda", torch.cuda.current_device())
+    cdt = torch.complex128 if spec["dtype"] == "c128" else torch.complex64
+    rdt = torch.float64 if spec["dtype"] == "c128" else torch.float32
+    cnt, dt, imag = w.schedule[0]
+    tau = 0.5 * dt
+    ny, nx = w.ny, w.nx
+    def field(f):
+        return torch.zeros((ny, nx), dtype=rdt, device=dev) if f is None else torch.from_numpy(np.ascontiguousarray(f)).to(dev, rdt)
+    V, Om, De = field(w.V), field(w.Omega), field(w.delta)
+    psi = torch.from_numpy(np.ascontiguousarray(np.moveaxis(w.psi0, 2, 0))).to(dev, cdt)  # [2, ny, nx]
+    kx = torch.from_numpy(2.0 * np.pi * np.fft.fftfreq(nx, d=w.Lx / nx)).to(dev)
+    ky = torch.from_numpy(2.0 * np.pi * np.fft.fftfreq(ny, d=w.Ly / ny)).to(dev)
+    K = torch.stack([0.5 * ((kx + w.k_L) ** 2)[None, :] + 0.5 * (ky ** 2)[:, None],
+                     0.5 * ((kx - w.k_L) ** 2)[None, :] + 0.5 * (ky ** 2)[:, None]])          # [2, ny, nx] fp64
+    kphase = (torch.exp(-K * dt) if imag else torch.exp(-1j * K * dt)).to(cdt)
+    cell = (w.Lx / nx) * (w.Ly / ny)
+    targets = cell * (psi.abs() ** 2).sum(dim=(1, 2))
+
+    def half(psi):
+        u, d = psi[0], psi[1]
+        nu, nd = u.real ** 2 + u.imag ** 2, d.real ** 2 + d.imag ** 2
+        d_up = V + w.g_uu * nu + w.g_ud * nd + 0.5 * De
+        d_dn = V + w.g_dd * nd + w.g_ud * nu - 0.5 * De
+        a, bz, bx = 0.5 * (d_up + d_dn), 0.5 * (d_up - d_dn), 0.5 * Om
+        th = torch.sqrt(bx * bx + bz * bz) * tau
+        if imag:
+            c = torch.cosh(th)
+            s = tau * torch.where(th.abs() < 1e-4, 1.0 + th * th / 6.0, torch.sinh(th) / th)
+            e = torch.exp(-a * tau)
+            return torch.stack([e * (c * u - s * (bz * u + bx * d)), e * (c * d - s * (bx * u - bz * d))])
+        c = torch.cos(th)
+        s = tau * torch.sinc(th / np.pi)          # sin(theta)/|b|
+        ph = torch.polar(torch.ones_like(a), -a * tau)
+        return torch.stack([ph * (c * u - 1j * s * (bz * u + bx * d)), ph * (c * d - 1j * s * (bx * u - bz * d))])
+
+    def step(psi):
+        psi = half(psi)
+        psi = torch.fft.ifft2(torch.fft.fft2(psi, dim=(1, 2)) * kphase, dim=(1, 2))
+        psi = half(psi)
+        if imag:
+            n = cell * (psi.abs() ** 2).sum(dim=(1, 2))
+            sc = torch.sqrt(targets / n) if w.norm_mode == 0 else torch.sqrt(targets.sum() / n.sum()).expand(2)
+            psi = psi * sc[:, None, None].to(rdt)
+        return psi
+
+    q = psi
+    for _ in range(warmup):
+        q = step(q)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    q = psi
+    e0.record()
+    for _ in range(steps):
+        q = step(q)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    out = {"kind": "torch.fft (cuFFT) + torch elementwise operations: the paper's formulation of the step, this GPU",
+           "ms_per_step": ms, "value": w.points / (ms * 1e-3), "unit": UNIT, "steps": steps,
+           "note": "context, not part of the product path; library calls only"}
+    if ours_after_steps is not None:
+        ref = np.moveaxis(q.cpu().numpy(), 0, 2).astype(np.complex128)
+        got = ours_after_steps.astype(np.complex128)
+        out["rel_l2_ours_vs_this"] = float(np.linalg.norm((got - ref).ravel()) / np.linalg.norm(ref.ravel()))
+    return out
 
 
 def whole_job_value(points: int, steps: int, ms_local: float, world: int, group=None):
@@ -371,6 +449,16 @@ def run_ours(args, wname):
                     "job": f"fields + psi host->device, spgpe_step({K}), psi device->host; {e2e_s:.4f} s"},
             "gpu_launches": int(launches), "clocks": clocks, "finite": finite, "norms": list(map(float, norms)),
         }
+        if world == 1 and not args.no_cufft and psi_bytes <= (1 << 28):
+            # context: the paper's formulation (torch.fft + elementwise torch operations) on this GPU, and a cross-check
+            # of the library against it after the same number of steps from the same initial state
+            n_cmp = min(K, 20)
+            h2 = sp.from_workload(w, stream=stream.cuda_stream)
+            sp.spgpe_step(h2, n_cmp, dt, imag)
+            ours_cmp = sp.spgpe_get_psi_host(h2)
+            sp.spgpe_destroy(h2)
+            line["cufft_comparison"] = cufft_comparison(w, spec, n_cmp, 3, ours_cmp)
+            line["cufft_comparison"]["ours_speedup"] = line["cufft_comparison"]["ms_per_step"] / (ms / K)
         if world == 1 and not args.no_cpu:
             v, cores, what, sec = oracle_sample(spec["cfg"], spec["dtype"], budget_s=20.0, steps=3)
             v1, _, what1, sec1 = oracle_sample(spec["cfg"], spec["dtype"], budget_s=10.0, steps=3, threads=1)
@@ -393,6 +481,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="4", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-cufft", action="store_true", help="skip the torch.fft / elementwise comparison leg")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
