@@ -229,9 +229,16 @@ static void fill_ktables(const spgpe_ctx* h, std::vector<double>& Kx, std::vecto
   Kx.resize(2 * (size_t)h->nx);
   Ky.resize(h->ny);
   kxv.resize(h->nx);
-  // unsplit axis: entry pos belongs to the frequency stored at pos; split axis: entry f belongs to frequency f
+  // unsplit axis: entry pos belongs to the frequency stored at pos.  Split axis (two sub-lines of m = n/2 points): entry
+  // i*m + pos belongs to the frequency f + i*m of the joined spectrum, f = frequency stored at position pos of a
+  // sub-transform -- the order in which the join kernel (split.cu) meets them, so that its table reads are coalesced
+  auto freq_of_entry = [](int n, int split, int e) {
+    if (split == 1) return plan_freq_of_pos(n, e);
+    const int m = n / split;
+    return plan_freq_of_pos(m, e % m) + (e / m) * m;
+  };
   for (int pos = 0; pos < h->nx; ++pos) {
-    const int f = h->sx == 1 ? plan_freq_of_pos(h->nx, pos) : pos;
+    const int f = freq_of_entry(h->nx, h->sx, pos);
     const int mt = (f < h->nx / 2) ? f : f - h->nx;
     const double k = two_pi * (double)mt / h->Lx;
     Kx[pos] = 0.5 * (k + h->p.k_L) * (k + h->p.k_L);
@@ -239,7 +246,7 @@ static void fill_ktables(const spgpe_ctx* h, std::vector<double>& Kx, std::vecto
     kxv[pos] = k;
   }
   for (int pos = 0; pos < h->ny; ++pos) {
-    const int f = h->sy == 1 ? plan_freq_of_pos(h->ny, pos) : pos;
+    const int f = freq_of_entry(h->ny, h->sy, pos);
     const int mt = (f < h->ny / 2) ? f : f - h->ny;
     const double k = two_pi * (double)mt / h->Ly;
     Ky[pos] = 0.5 * k * k;

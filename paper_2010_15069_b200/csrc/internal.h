@@ -43,9 +43,9 @@ struct SplitArgs {
   const int* fy;       // [ny/2]
   const double2* wx;   // [nx/2] exp(-2 pi i fx[pos] / nx)
   const double2* wy;   // [ny/2]
-  const double2* phx;  // [2][nx] k_x phase: by true frequency (split x axis) or by stored position (unsplit)
-  const double2* phy;  // [ny]    k_y phase by true frequency, 1/(nx ny) included (split y axis only)
-  const double* Kx;    // [2][nx] energy mode: by true frequency (split axis) or by stored position (unsplit)
+  const double2* phx;  // [2][nx] k_x phase: entry i*mx + pos of the join (split x axis) or stored position (unsplit)
+  const double2* phy;  // [ny]    k_y phase, entry j*my + pos of the join, 1/(nx ny) included (split y axis only)
+  const double* Kx;    // [2][nx] energy mode: same order as phx
   const double* Ky;    // [ny]
   double* partial;     // [gridDim.x] energy mode
 };

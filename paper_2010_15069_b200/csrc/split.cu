@@ -37,9 +37,8 @@ __global__ void __launch_bounds__(256) split_kernel(const SplitArgs a) {
           for (int c = 0; c < 2; ++c) u[j][i][c] = St::ld(a.psi, pt * 2 + c);
         }
       }
-    // true frequencies of the block: f + ax m along a split axis; along an unsplit axis the stored position itself
-    // indexes the (stored-order) tables
-    const int fx = SX == 2 ? a.fx[px] : px, fy = SY == 2 ? a.fy[py] : py;
+    // the tables of a split axis are stored in the order of the join (api.cu, fill_ktables): entry i*m + pos
+    const int fx = px, fy = py;
     if (SX == 2) {
       const double2 w = a.wx[px];
 #pragma unroll
@@ -74,7 +73,7 @@ __global__ void __launch_bounds__(256) split_kernel(const SplitArgs a) {
           }
       continue;
     }
-    {  // k_x phase: by true frequency along a split x axis, by stored position (fx = px, i = 0) along an unsplit one
+    {  // k_x phase: entry px + i*mx along a split x axis, stored position (i = 0) along an unsplit one
 #pragma unroll
       for (int j = 0; j < SY; ++j)
 #pragma unroll
