@@ -232,7 +232,10 @@ def test_fp32_and_fp64_arithmetic_kernels_agree_and_mix(sp, monkeypatch):
 
 
 @pytest.mark.parametrize("split_min,nx,ny", [(128, 128, 256), (128, 1024, 64), (1024, 1024, 1024), (1024, 2048, 256),
-                                             (1024, 64, 1024)])
+                                             (1024, 64, 1024),
+                                             # longer sub-lines and mixed cases
+                                             (2048, 64, 2048), (2048, 2048, 2048), (512, 512, 512), (256, 64, 512),
+                                             (4096, 128, 4096)])
 @pytest.mark.parametrize("imag", [0, 1])
 def test_fp32_path_with_split_axes(sp, monkeypatch, split_min, nx, ny, imag):
     """Split axes of complex64 grids (SPGPE_DEBUG_SPLIT_MIN forces them at small sizes): sub-lines of 512 points and
