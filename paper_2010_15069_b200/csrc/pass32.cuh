@@ -166,6 +166,7 @@ __global__ void __launch_bounds__(LINES * (NX / 16), (LINES * (NX / 16) <= 128) 
   double su = 0.0, sd = 0.0;
   cf u[16], d[16];
   int it = 0;
+  TL_DECL(8);
   for (int grp = blockIdx.x; grp < ngroups; ++it) {
     if (tid == 0) {
       next_s[it & 1] = nxt;
@@ -179,6 +180,7 @@ __global__ void __launch_bounds__(LINES * (NX / 16), (LINES * (NX / 16) <= 128) 
       }
     }
     mbar_wait(&full, it & 1);
+    TL_MARK(0);
     {
 #pragma unroll
       for (int n = 0; n < 16; ++n) {
@@ -217,11 +219,15 @@ __global__ void __launch_bounds__(LINES * (NX / 16), (LINES * (NX / 16) <= 128) 
           for (int k = tid; k < (int)(FIELD_BYTES / 16); k += NTHR) z[k] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
     };
+    TL_MARK(1);
     if (MODE == MODE_MID || MODE == MODE_EPI) line_inv32<NX, LINEW, LASTW>(buf, twS, t, u, d, fields_hook);
     else fields_hook();
+    TL_MARK(2);
     mbar_wait(&ffull, it & 1);
+    TL_MARK(3);
     if (a.V == nullptr || a.Om == nullptr || a.De == nullptr) __syncthreads();  // zero fills are per-thread writes
     real_space32<NX, LINES, MODE, XS>(u, d, a, fbuf, line, t, lc, su, sd);
+    TL_MARK(4);
     if (MODE == MODE_EPI && a.want_norm) {
 #pragma unroll
       for (int m = 16; m >= 1; m >>= 1) {
@@ -242,6 +248,7 @@ __global__ void __launch_bounds__(LINES * (NX / 16), (LINES * (NX / 16) <= 128) 
     if (MODE != MODE_EPI) {
       fwd_stages32<NX, 1, LINEW, LASTW>(buf, twS, t, u, d);
       __syncthreads();  // the last exchange has been read by every warp: the line buffers are free
+      TL_MARK(5);
     }
     const int nxt_grp = next_s[it & 1];
     if (tid == 0 && nxt_grp < ngroups) {
@@ -262,8 +269,11 @@ __global__ void __launch_bounds__(LINES * (NX / 16), (LINES * (NX / 16) <= 128) 
         dst[XS == 1 ? line * NX + x : 2 * x + line] = make_float4(u[n].re, u[n].im, d[n].re, d[n].im);
       }
     }
+    TL_MARK(6);
+    TL_TILE();
     grp = nxt_grp;
   }
+  if (MODE == MODE_MID) TL_DUMP("row32 wait|stage|inv|fieldwait|real|fwd|last+store", 7);
   if (MODE == MODE_EPI) {
     __shared__ int last_s;
     if (tid == 0) last_s = sched_finish(a.sched) ? 1 : 0;
