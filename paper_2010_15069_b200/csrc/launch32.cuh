@@ -9,7 +9,7 @@ template <int N, int MODE, int XS>
 cudaError_t launch_row32_xs(const PassXArgs& a, int ny, cudaStream_t s, const LaunchEnv& env, int* grid_out) {
   constexpr int L = (XS == 2) ? 2 : Lines32<N>::X;
   auto k = row32_kernel<N, L, MODE, XS>;
-  constexpr size_t smem = Smem32<N, L>::BYTES_X;
+  constexpr size_t smem = (XS == 2) ? Smem32<N, L>::BYTES_Y : Smem32<N, L>::BYTES_X;
   static int cache[SPGPE_MAX_DEVICES] = {};
   int resident = 0;
   cudaError_t e = resident_ctas(k, L * (N / 16), smem, env, cache, &resident);

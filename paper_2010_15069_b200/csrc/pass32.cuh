@@ -130,10 +130,13 @@ __global__ void __launch_bounds__(LINES * (NX / 16), (LINES * (NX / 16) <= 128) 
   constexpr bool LASTW = LINEW || P::NS == 3;   // the RL threads of a block are consecutive t: one warp
   static_assert(NTHR % 32 == 0 && 32 % (T < 32 ? T : 32) == 0, "lines must not straddle warps");
   const int tid = threadIdx.x;
-  const int t = tid % T;
-  const int line = tid / T;
-  float4* buf = smem4 + (size_t)line * SM::LSTRIDE_X;
-  float4* twS = smem4 + SM::EBUF_X;
+  // XS == 1: a line (row) per group of T consecutive threads.  XS == 2: the even and the odd points of one row sit in
+  // ADJACENT lanes (column-style mapping, line buffers LSTRIDE_Y apart): a lane pair then reads and writes one 32-byte
+  // piece of the row (with the two lines in different warps every store was a 16-byte piece at a 32-byte pitch)
+  const int t = (XS == 2) ? tid / 2 : tid % T;
+  const int line = (XS == 2) ? tid % 2 : tid / T;
+  float4* buf = smem4 + (size_t)line * (XS == 2 ? SM::LSTRIDE_Y : SM::LSTRIDE_X);
+  float4* twS = smem4 + (XS == 2 ? SM::EBUF_Y : SM::EBUF_X);
   const float4* stg = smem4;                                    // staged rows, dense: [line][x]
   const float* fbuf = reinterpret_cast<const float*>(smem4);    // staged fields: [field][line][x]
   const int ngroups = a.ny / LINES;
