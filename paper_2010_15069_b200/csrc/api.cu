@@ -49,6 +49,7 @@ struct spgpe_ctx {
   CUtensorMap tmap_psi, tmap_scratch, tmap_psi_db, tmap_psi32;  // column-pass tensor maps of psi / the energy scratch buffer
   int* sched;    // [4] work counters of the persistent kernels: row pass [0..1], column pass [2..3]
   double2 *wcx, *wcy;         // split axes: join twiddles
+  float4 *wcx32, *wcy32;      // ... as two-float values (fp32 join of complex64 storage)
   int *fpx, *fpy;             // split axes: true frequency of a sub-transform position
   double* fmax;  // [3] max |V|, |Omega|, |delta| (tier bounds of the row pass)
   int partial_cap;
@@ -372,6 +373,14 @@ extern "C" int spgpe_create(spgpe_handle* out, int nx, int ny, double Lx, double
     alloc((void**)dwc, sizeof(double2) * m);
     if (e == cudaSuccess) e = cudaMemcpy(*dfp, fp.data(), sizeof(int) * m, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(*dwc, wc.data(), sizeof(double2) * m, cudaMemcpyHostToDevice);
+    std::vector<float4> wc32(m);
+    for (int pos = 0; pos < m; ++pos) {
+      const float hr = (float)wc[pos].x, hi = (float)wc[pos].y;
+      wc32[pos] = make_float4(hr, hi, (float)(wc[pos].x - (double)hr), (float)(wc[pos].y - (double)hi));
+    }
+    float4** dwc32 = ax ? &h->wcy32 : &h->wcx32;
+    alloc((void**)dwc32, sizeof(float4) * m);
+    if (e == cudaSuccess) e = cudaMemcpy(*dwc32, wc32.data(), sizeof(float4) * m, cudaMemcpyHostToDevice);
   }
   if (e == cudaSuccess) e = make_col_tmap(h, h->psi, plan_lines_y(h->my), &h->tmap_psi);
   if (e == cudaSuccess && h->f32_ok) e = make_col_tmap(h, h->psi, plan_lines_y32(h->my), &h->tmap_psi32);
@@ -389,7 +398,7 @@ extern "C" int spgpe_destroy(spgpe_handle h) {
   ON_DEVICE(h);
   cudaStreamSynchronize(h->stream);
   void* ptrs[] = {h->psi, h->scratch, h->Vbuf, h->Ombuf, h->Debuf, h->tw_x, h->tw_y, h->Kx, h->Ky, h->kxv, h->kpartial,
-                  h->exk, h->eyk, h->exk32, h->eyk32, h->tw_x32, h->tw_y32, h->partial, h->scale, h->target, h->dout, h->fmax, h->sched, h->wcx, h->wcy, h->fpx, h->fpy};
+                  h->exk, h->eyk, h->exk32, h->eyk32, h->tw_x32, h->tw_y32, h->partial, h->scale, h->target, h->dout, h->fmax, h->sched, h->wcx, h->wcy, h->wcx32, h->wcy32, h->fpx, h->fpy};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   if (h->prof_ev) {
@@ -491,6 +500,7 @@ static SplitArgs split_args(spgpe_ctx* h, void* psi) {
   memset(&sa, 0, sizeof(sa));
   sa.psi = psi; sa.nx = h->nx; sa.ny = h->ny; sa.fx = h->fpx; sa.fy = h->fpy; sa.wx = h->wcx; sa.wy = h->wcy;
   sa.phx = h->exk; sa.phy = h->eyk; sa.Kx = h->Kx; sa.Ky = h->Ky; sa.partial = h->partial;
+  if (h->f32_ok && h->f32_dbg == 0) { sa.wx32 = h->wcx32; sa.wy32 = h->wcy32; sa.phx32 = h->exk32; sa.phy32 = h->eyk32; }
   return sa;
 }
 

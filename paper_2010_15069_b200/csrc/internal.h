@@ -48,6 +48,8 @@ struct SplitArgs {
   const double* Kx;    // [2][nx] energy mode: same order as phx
   const double* Ky;    // [ny]
   double* partial;     // [gridDim.x] energy mode
+  // two-float copies of wx, wy, phx, phy for the fp32 join of complex64 storage (split32_kernel); NULL: fp64 arithmetic
+  const float4 *wx32, *wy32, *phx32, *phy32;
 };
 cudaError_t launch_split(int dt, const SplitArgs& a, int sx, int sy, int energy, int nblk, cudaStream_t s);
 

@@ -11,6 +11,7 @@
 // one (pos_x, pos_y) and both components, so the step is local and in place.
 // MODE_ENERGY instead accumulates sum (Kx_c + Ky) |X|^2 (spgpe_energy) and writes nothing back.
 #include "internal.h"
+#include "fft32.cuh"
 
 namespace spgpe {
 
@@ -144,6 +145,89 @@ __global__ void __launch_bounds__(256) split_kernel(const SplitArgs a) {
   }
 }
 
+// The same join for complex64 storage in the arithmetic of the fp32 transforms (fft32.cuh, R-14): fp32
+// butterflies, every fixed factor (join twiddles, k-space phases) as a two-float value.  One thread owns the SX x SY
+// block of one (pos_x, pos_y), both components of a point in one 16-byte access.
+template <int SX, int SY>
+__global__ void __launch_bounds__(256) split32_kernel(const SplitArgs a) {
+  const int mx = a.nx / SX, my = a.ny / SY;
+  float4* psi = reinterpret_cast<float4*>(a.psi);
+  for (size_t b = (size_t)blockIdx.x * blockDim.x + threadIdx.x; b < (size_t)mx * my;
+       b += (size_t)gridDim.x * blockDim.x) {
+    const int px = (int)(b % mx), py = (int)(b / mx);
+    cf u[SY][SX], d[SY][SX];
+#pragma unroll
+    for (int j = 0; j < SY; ++j)
+#pragma unroll
+      for (int i = 0; i < SX; ++i) {
+        const float4 q = __ldcs(psi + ((size_t)py * SY + j) * a.nx + (size_t)px * SX + i);
+        u[j][i] = mkf(q.x, q.y);
+        d[j][i] = mkf(q.z, q.w);
+      }
+    float4 wx = make_float4(1.f, 0.f, 0.f, 0.f), wy = wx;
+    if (SX == 2) {
+      wx = __ldg(a.wx32 + px);
+#pragma unroll
+      for (int j = 0; j < SY; ++j) {
+        const cf ou = cmul2(u[j][1], wx.x, wx.y, wx.z, wx.w), od = cmul2(d[j][1], wx.x, wx.y, wx.z, wx.w);
+        const cf eu = u[j][0], ed = d[j][0];
+        u[j][0] = eu + ou; u[j][1] = eu - ou;
+        d[j][0] = ed + od; d[j][1] = ed - od;
+      }
+    }
+    if (SY == 2) {
+      wy = __ldg(a.wy32 + py);
+#pragma unroll
+      for (int i = 0; i < SX; ++i) {
+        const cf ou = cmul2(u[1][i], wy.x, wy.y, wy.z, wy.w), od = cmul2(d[1][i], wy.x, wy.y, wy.z, wy.w);
+        const cf eu = u[0][i], ed = d[0][i];
+        u[0][i] = eu + ou; u[1][i] = eu - ou;
+        d[0][i] = ed + od; d[1][i] = ed - od;
+      }
+    }
+    // k_x phase (entry px + i*mx; stored position for an unsplit x axis), k_y phase of a split y axis (entry py + j*my)
+#pragma unroll
+    for (int i = 0; i < SX; ++i) {
+      const float4 fu = __ldg(a.phx32 + px + i * mx), fd = __ldg(a.phx32 + (size_t)a.nx + px + i * mx);
+#pragma unroll
+      for (int j = 0; j < SY; ++j) {
+        u[j][i] = cmul2(u[j][i], fu.x, fu.y, fu.z, fu.w);
+        d[j][i] = cmul2(d[j][i], fd.x, fd.y, fd.z, fd.w);
+      }
+    }
+    if (SY == 2) {
+#pragma unroll
+      for (int j = 0; j < SY; ++j) {
+        const float4 f = __ldg(a.phy32 + py + j * my);
+#pragma unroll
+        for (int i = 0; i < SX; ++i) {
+          u[j][i] = cmul2(u[j][i], f.x, f.y, f.z, f.w);
+          d[j][i] = cmul2(d[j][i], f.x, f.y, f.z, f.w);
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < SX; ++i) {
+        const cf su = u[0][i] + u[1][i], du = u[0][i] - u[1][i], sd = d[0][i] + d[1][i], dd = d[0][i] - d[1][i];
+        u[0][i] = su; u[1][i] = cmul2c(du, wy.x, wy.y, wy.z, wy.w);
+        d[0][i] = sd; d[1][i] = cmul2c(dd, wy.x, wy.y, wy.z, wy.w);
+      }
+    }
+    if (SX == 2) {
+#pragma unroll
+      for (int j = 0; j < SY; ++j) {
+        const cf su = u[j][0] + u[j][1], du = u[j][0] - u[j][1], sd = d[j][0] + d[j][1], dd = d[j][0] - d[j][1];
+        u[j][0] = su; u[j][1] = cmul2c(du, wx.x, wx.y, wx.z, wx.w);
+        d[j][0] = sd; d[j][1] = cmul2c(dd, wx.x, wx.y, wx.z, wx.w);
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < SY; ++j)
+#pragma unroll
+      for (int i = 0; i < SX; ++i)
+        psi[((size_t)py * SY + j) * a.nx + (size_t)px * SX + i] = make_float4(u[j][i].re, u[j][i].im, d[j][i].re, d[j][i].im);
+  }
+}
+
 template <int DT, bool ENERGY>
 static cudaError_t launch_split_dt(const SplitArgs& a, int sx, int sy, int nblk, cudaStream_t s) {
   if (sx == 2 && sy == 2) split_kernel<DT, 2, 2, ENERGY><<<nblk, 256, 0, s>>>(a);
@@ -156,6 +240,12 @@ static cudaError_t launch_split_dt(const SplitArgs& a, int sx, int sy, int nblk,
 // nblk CTAs of 256 threads; with energy != 0 partial[nblk] receives the per-CTA sums
 cudaError_t launch_split(int dt, const SplitArgs& a, int sx, int sy, int energy, int nblk, cudaStream_t s) {
   if (dt == 0) return energy ? launch_split_dt<0, true>(a, sx, sy, nblk, s) : launch_split_dt<0, false>(a, sx, sy, nblk, s);
+  if (!energy && a.phx32 != nullptr) {  // complex64 storage, step: fp32 arithmetic with two-float factors
+    if (sx == 2 && sy == 2) split32_kernel<2, 2><<<nblk, 256, 0, s>>>(a);
+    else if (sx == 2) split32_kernel<2, 1><<<nblk, 256, 0, s>>>(a);
+    else split32_kernel<1, 2><<<nblk, 256, 0, s>>>(a);
+    return cudaGetLastError();
+  }
   return energy ? launch_split_dt<1, true>(a, sx, sy, nblk, s) : launch_split_dt<1, false>(a, sx, sy, nblk, s);
 }
 
