@@ -381,7 +381,24 @@ __global__ void __launch_bounds__(LINES * (NY / 16), (LINES * (NY / 16) <= 256) 
       lds4(stg, (YMODE == YMODE_INVONLY ? stored_pos32<NY>(t, n) : t + n * T) * LINES + line, u[n], d[n]);
     __syncthreads();  // every thread has taken its staged values: the buffers may be overwritten
     TL_MARK(1);
-    if (YMODE != YMODE_INVONLY) line_fwd32<NY, LINEW, LASTW>(buf, twS, t, u, d);
+    int nxt_grp = ngroups;
+    auto hook = [&]() {
+      __syncthreads();  // last read of the line buffers done by every warp: the next tile may land
+      nxt_grp = next_s[it & 1];
+      if (tid == 0 && nxt_grp < ngroups) {
+        issue_loads(nxt_grp);
+        nxt = sched_next(a.sched);
+      }
+    };
+    if (YMODE == YMODE_FWDONLY) {
+      // the line buffers are free behind the last exchange: the next tile's load runs under the last butterflies too
+      fwd_stages32<NY, 1, LINEW, LASTW>(buf, twS, t, u, d);
+      hook();
+      dft_lastf<-1, P::RL>(u);
+      dft_lastf<-1, P::RL>(d);
+    } else if (YMODE != YMODE_INVONLY) {
+      line_fwd32<NY, LINEW, LASTW>(buf, twS, t, u, d);
+    }
     TL_MARK(2);
     if (YMODE == YMODE_STEP) {
       const bool has_x = a.exk32 != nullptr;
@@ -399,18 +416,8 @@ __global__ void __launch_bounds__(LINES * (NY / 16), (LINES * (NY / 16) <= 256) 
       }
     }
     TL_MARK(3);
-    int nxt_grp = ngroups;
-    auto hook = [&]() {
-      __syncthreads();  // last read of the line buffers done by every warp: the next tile may land
-      nxt_grp = next_s[it & 1];
-      if (tid == 0 && nxt_grp < ngroups) {
-        issue_loads(nxt_grp);
-        nxt = sched_next(a.sched);
-      }
-    };
     float4* dst = reinterpret_cast<float4*>(a.psi) + col;
     if (YMODE == YMODE_FWDONLY) {
-      hook();
 #pragma unroll
       for (int n = 0; n < 16; ++n)
         dst[(size_t)stored_pos32<NY>(t, n) * a.nx] = make_float4(u[n].re, u[n].im, d[n].re, d[n].im);
