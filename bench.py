@@ -364,6 +364,20 @@ def run_ours(args, wname):
     launches = (sp.spgpe_launch_count(h) - l0) // args.repeats
     ms = float(np.median(region_ms))
     mad_ms = float(np.median(np.abs(np.array(region_ms) - ms)))
+    # ---- optional: the same K steps replayed from a CUDA graph of one captured spgpe_step(K) call -----------
+    graph_leg = None
+    if args.graph:
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(stream):
+            with torch.cuda.graph(g, stream=stream):
+                sp.spgpe_step(h, K, dt, imag)
+        g_ms = [timed_region(lambda: g.replay()) for _ in range(args.repeats)]
+        gm = float(np.median(g_ms))
+        graph_leg = {"ms_per_step": gm / K, "ms_per_step_mad": float(np.median(np.abs(np.array(g_ms) - gm))) / K,
+                     "ms_per_step_all": [m / K for m in g_ms],
+                     "note": "the caller captured one spgpe_step(K) call (stream capture) and replays it; "
+                             "context, `value` is the plain call's"}
+        del g
     # ---- per-launch durations of the two pass kernels (second region of K steps) -----------------------
     sp.spgpe_profile(h, True)
     sp.spgpe_step(h, K, dt, imag)
@@ -449,6 +463,8 @@ def run_ours(args, wname):
                     "job": f"fields + psi host->device, spgpe_step({K}), psi device->host; {e2e_s:.4f} s"},
             "gpu_launches": int(launches), "clocks": clocks, "finite": finite, "norms": list(map(float, norms)),
         }
+        if graph_leg is not None:
+            line["graph_replay"] = graph_leg
         if world == 1 and not args.no_cufft and psi_bytes <= (1 << 28):
             # context: the paper's formulation (torch.fft + elementwise torch operations) on this GPU, and a cross-check
             # of the library against it after the same number of steps from the same initial state
@@ -481,6 +497,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="4", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--graph", action="store_true",
+                    help="also time replays of a CUDA graph of one captured spgpe_step(K) call (graph_replay)")
     ap.add_argument("--no-cufft", action="store_true", help="skip the torch.fft / elementwise comparison leg")
     args = ap.parse_args()
     if args.warmup < 3:

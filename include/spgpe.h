@@ -91,7 +91,14 @@ int spgpe_set_norm_targets(spgpe_handle h, double n_up, double n_dn);
 /* n Strang steps of size dt.  imag != 0: imaginary time with dt = d tau > 0 and a
  * renormalisation after every step.  dt may be negative in real time; NaN or infinite dt, and dt <= 0 in imaginary
  * time, return SPGPE_ERR_INVALID_ARG.  A component whose norm is zero keeps scale 1 (it stays zero).  Asynchronous.
- * step(n) then step(m) equals step(n+m) to rounding. */
+ * step(n) then step(m) equals step(n+m) to rounding.
+ * Stream capture: the call only enqueues kernels on the handle's stream (no allocation, no synchronisation, no host
+ * read-back; the imaginary-time rescale factors travel through device memory), so a caller may record it into a CUDA
+ * graph (cudaStreamBeginCapture on that stream) and replay the graph; every replay advances the state by n steps,
+ * bit-identical with the plain call (tests/test_gpu_graph.py).  Two conditions: the k-space tables of (dt, imag) are
+ * built by the first call that uses them, so one plain call with the same (dt, imag) precedes the capture; and an
+ * annealed schedule (spgpe_set_annealing) fixes its event indices at capture time and must not be replayed.
+ * spgpe_profile must be off during a capture. */
 int spgpe_step(spgpe_handle h, int n, double dt, int imag);
 
 /* Form of the real-space part R(tau) used by later steps (host-side switch, no device work):
