@@ -488,6 +488,78 @@ def run_ours(args, wname):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """The paper's own benchmark (Figure 2): evaluation time of the stepping function against the
+    grid size N = Nx Ny = 2^eta (N = points of one component), complex128, median and median absolute deviation over
+    repeated timings, and the linear fit t(N) = theta N + xi the paper reports for its GPUs (theta = 9.7e-8 s per point).
+    Config 4's recipe (all terms on, real time) on nx = 2^ceil(eta/2), ny = 2^floor(eta/2): square grids for even eta,
+    2:1 grids for odd eta.  Two times per size: one spgpe_step(1) call (what the paper's timeit measures: a whole
+    call, opening + column + closing pass) and the per-step time inside one spgpe_step(K) call (steady state)."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libspgpe has no CPU fallback")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import paper_2010_15069_b200 as sp
+    import workloads as wl
+    sp.lib()
+    stream = torch.cuda.Stream()
+    rows = []
+
+    def region(fn):
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            fn()
+            e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e-3
+
+    def med_mad(v):
+        m = float(np.median(v))
+        return m, float(np.median(np.abs(np.array(v) - m)))
+
+    for eta in range(args.eta_min, args.eta_max + 1):
+        nx, ny = 1 << ((eta + 1) // 2), 1 << (eta // 2)
+        w = wl.make_workload(4, dtype="c128", nx=nx, ny=ny)
+        _, dt, imag = w.schedule[0]
+        h = sp.from_workload(w, stream=stream.cuda_stream)
+        sp.spgpe_step(h, max(3, args.warmup), dt, imag)
+        sp.spgpe_synchronize(h)
+        sampler = ClockSampler(0)  # per size: the host-side generation of the next grid leaves the GPU idle
+        sampler.start()
+        t10 = region(lambda: sp.spgpe_step(h, 10, dt, imag)) / 10
+        K = int(min(2000, max(10, 0.05 / t10)))  # regions of about 50 ms
+        one, one_mad = med_mad([region(lambda: sp.spgpe_step(h, 1, dt, imag)) for _ in range(max(args.repeats, 21))])
+        many, many_mad = med_mad([region(lambda: sp.spgpe_step(h, K, dt, imag)) / K for _ in range(args.repeats)])
+        clocks = sampler.stop()
+        norms = sp.spgpe_norm(h)
+        rows.append({"eta": eta, "grid": [nx, ny], "points": nx * ny, "one_step_call_s": one, "one_step_call_mad_s": one_mad,
+                     "steps_per_region": K, "s_per_step": many, "s_per_step_mad": many_mad,
+                     "finite": bool(np.isfinite(norms).all()), "clocks": clocks})
+        sp.spgpe_destroy(h)
+        del w
+    N = np.array([r["points"] for r in rows], dtype=np.float64)
+    A = np.stack([N, np.ones_like(N)], axis=1)
+
+    def fit(key):
+        th, xi = np.linalg.lstsq(A, np.array([r[key] for r in rows]), rcond=None)[0]
+        return {"theta_s_per_point": float(th), "xi_s": float(xi)}
+
+    print(json.dumps({
+        "metric": "step evaluation time against grid size, t(N) = theta N + xi", "unit": "s", "dtype": "f64",
+        "data": "synthetic", "n_gpus": 1, "higher_is_better": False,
+        "config": {"workload": "config 4 recipe (complex128, real time, all terms on) at N = 2^eta points per component, "
+                               "nx = 2^ceil(eta/2), ny = 2^floor(eta/2)", "eta": [args.eta_min, args.eta_max],
+                   "repeats": args.repeats, "l2": "sizes up to eta = 21 fit the 126 MB L2, larger ones do not; no flush"},
+        "sweep": rows, "fit_one_step_call": fit("one_step_call_s"), "fit_steady_state": fit("s_per_step"),
+        "paper": {"theta_s_per_point": 9.7e-8, "where": "PAPER.md L189 (Figure 2): the paper's GPUs (MX150, GTX 980 Ti, "
+                  "Titan V), PyTorch + cuFFT, complex128; another machine's number: context, not the target"}}),
+          flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -500,11 +572,19 @@ def main():
     ap.add_argument("--graph", action="store_true",
                     help="also time replays of a CUDA graph of one captured spgpe_step(K) call (graph_replay)")
     ap.add_argument("--no-cufft", action="store_true", help="skip the torch.fft / elementwise comparison leg")
+    ap.add_argument("--sweep", action="store_true",
+                    help="the paper's Figure 2 instead of the headline line: step time against N = 2^eta (complex128)")
+    ap.add_argument("--eta-min", type=int, default=12)
+    ap.add_argument("--eta-max", type=int, default=24)
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
     args.repeats = max(1, args.repeats)
-    if args.impl == "reference":
+    if args.sweep:
+        if not (12 <= args.eta_min <= args.eta_max <= 26):
+            ap.error("--eta-min / --eta-max: 12 <= eta <= 26 (line lengths 64 ... 8192)")
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args, args.workload)
     else:
         run_ours(args, args.workload)

@@ -24,3 +24,12 @@ def test_default_workload_is_the_metric_config():
     import bench
     assert bench.WORKLOADS["4"] == dict(cfg=4, dtype="c128")
     assert bench.METRIC.startswith("split-step")
+
+
+def test_sweep_rejects_sizes_outside_the_supported_line_lengths():
+    """--sweep (the paper's Figure 2: step time against N = 2^eta) takes 12 <= eta <= 26 only; the
+    argument check runs before any GPU work."""
+    for extra in (["--eta-max", "27"], ["--eta-min", "11"], ["--eta-min", "20", "--eta-max", "19"]):
+        r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--sweep"] + extra, capture_output=True,
+                           text=True, timeout=300, cwd=ROOT)
+        assert r.returncode == 2 and "eta" in r.stderr
