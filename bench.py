@@ -535,9 +535,16 @@ def run_sweep(args):
         one, one_mad = med_mad([region(lambda: sp.spgpe_step(h, 1, dt, imag)) for _ in range(max(args.repeats, 21))])
         many, many_mad = med_mad([region(lambda: sp.spgpe_step(h, K, dt, imag)) / K for _ in range(args.repeats)])
         clocks = sampler.stop()
+        # per-launch durations of the two pass kernels between events (serialised: no overlap of successive kernels)
+        sp.spgpe_profile(h, True)
+        sp.spgpe_step(h, min(K, 100), dt, imag)
+        kms, kcnt = sp.spgpe_profile_read(h)
+        sp.spgpe_profile(h, False)
         norms = sp.spgpe_norm(h)
         rows.append({"eta": eta, "grid": [nx, ny], "points": nx * ny, "one_step_call_s": one, "one_step_call_mad_s": one_mad,
                      "steps_per_region": K, "s_per_step": many, "s_per_step_mad": many_mad,
+                     "serialised_launch_s": {"row_pass": kms[0] / max(kcnt[0], 1) * 1e-3,
+                                             "column_pass": kms[1] / max(kcnt[1], 1) * 1e-3},
                      "finite": bool(np.isfinite(norms).all()), "clocks": clocks})
         sp.spgpe_destroy(h)
         del w
