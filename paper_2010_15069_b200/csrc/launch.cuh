@@ -10,9 +10,11 @@ namespace spgpe {
 // lines (rows or columns) per CTA: at most 256 threads per CTA up to N = 2048, 512 at N = 4096.  Rows of 512 points go two
 // to a CTA (128 threads, like the four rows of 256 points): with four (256 threads at 128 registers) the back-to-back
 // step at 512 x 256 / 512 x 512 was as long as the two serialised launches (25.1 / 32.1 us against 18.0 / 25.2 us with
-// two: profiles/r2_eta_sweep.md)
+// two: profiles/r2_eta_sweep.md).  Rows of 1024 points go one to a CTA (128 threads; with two, 1024 x 1024 took 35.2 us per
+// row pass against 31.0 us: config 3 73.0 -> 69.6 us/step).  Columns of 512 points stay four to a CTA (two: better at
+// 512 x 512 and 2048 x 512, worse at 1024 x 512); one row of 512 points per CTA is no better than two.
 template <int N> struct Lines {
-  static constexpr int X = (N >= 2048) ? 1 : (N >= 512 ? 2 : 4);
+  static constexpr int X = (N >= 1024) ? 1 : (N >= 512 ? 2 : 4);
   static constexpr int Y = (N >= 4096) ? 1 : (N >= 1024 ? 2 : 4);
   static constexpr int YDB = (N == 2048) ? 1 : (N == 1024 ? 2 : 0);  // columns per tile of pass_y_db_kernel (0: none)
 };
